@@ -1,0 +1,131 @@
+/*
+ * ljmd.h -- C ABI of the B200-native Lennard-Jones MD hot path of arXiv 0709.3225
+ * ("Harvesting graphics power for MD simulations"): one velocity-Verlet step with the
+ * force evaluated as all-pairs O(N^2) or through a cell list, and the rand48 generator
+ * with skip-ahead.  Citations are PAPER.md:<line> in /root/reference; "R<n>" are the
+ * numbered readings in DESIGN.md section 3.
+ *
+ * Conventions for every call
+ *   - Returns MD_OK (0) or a negative md_status; never aborts, never throws.
+ *   - Every array pointer is owned by the caller, may be HOST or DEVICE memory (detected
+ *     with cudaPointerGetAttributes), and is not retained after the call returns.
+ *   - Calls are synchronous for the caller: results are complete on return.  Kernels run
+ *     on the stream set with md_set_stream (default: the legacy default stream).
+ *   - A handle is not thread-safe; distinct handles are independent.
+ *   - Everything executes on the current CUDA device in sm_100a kernels.  There is no CPU
+ *     fallback: without a usable device every call returns MD_ECUDA.
+ *   - Reduced units, mass = 1, cubic periodic box [0,L)^3, minimum image (R3).
+ */
+#ifndef LJMD_H
+#define LJMD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct md_sim md_sim; /* opaque, created and destroyed by the library */
+
+typedef enum md_status {
+    MD_OK = 0,
+    MD_EINVAL = -1,       /* null pointer, non-positive size, unknown enum, rc > L/2, bad seed */
+    MD_EDOMAIN = -2,      /* algo = MD_CELL with fewer than 3 cells per dimension */
+    MD_ESTATE = -3,       /* step/get before md_set_state, or getters on stale forces */
+    MD_ENOMEM = -4,       /* device or host allocation failed */
+    MD_ECUDA = -5,        /* CUDA runtime error; see md_last_cuda_error */
+    MD_EUNSUPPORTED = -6  /* valid request that this build does not implement */
+} md_status;
+
+enum { MD_ALLPAIRS = 0, MD_CELL = 1 };                       /* algo */
+enum { MD_TRUNCATED = 0, MD_ENERGY_SHIFTED = 1, MD_FORCE_SHIFTED = 2 }; /* shifted */
+enum { R48_U32_HI32 = 0, R48_U32_HI31 = 1, R48_F64 = 2, R48_U64_STATE = 3 }; /* kind */
+
+/* Create a simulation of N atoms in a cubic periodic box of side L with the Lennard-Jones
+ * pair force of PAPER.md:56 (Eq. 2, with the 1/sigma factor of R1) cut at rc (strict r < rc,
+ * PAPER.md:61).  shifted: 0 truncated only; 1 energy-shifted, U(rc) = 0, force unshifted
+ * (the graded mode, R2); 2 the paper's force-shifted Eq. 3.  dt is the
+ * velocity-Verlet time step.  The box used is (double)(float)L (R13).
+ * Errors: MD_EINVAL for out == NULL, N <= 0, L <= 0, rc <= 0, eps < 0, sigma <= 0, dt <= 0,
+ * unknown shifted, or rc > L/2 (minimum image invalid); MD_ENOMEM; MD_ECUDA. */
+int md_create(md_sim **out, int64_t N, double L, double rc, double eps, double sigma,
+              double dt, int shifted);
+
+/* Free the handle and all device memory it owns.  md_destroy(NULL) is MD_OK. */
+int md_destroy(md_sim *s);
+
+/* Set positions and velocities, [N][3] floats xyz, host or device.  Positions are wrapped
+ * into [0,L) (R14).  Marks forces stale.  Atom i of these arrays is "atom i" for every
+ * getter, whatever internal order the library keeps. */
+int md_set_state(md_sim *s, const float *pos, const float *vel);
+
+/* Read back positions and velocities in the caller's atom order; either may be NULL. */
+int md_get_state(md_sim *s, float *pos, float *vel);
+
+/* Evaluate F, PE and the virial at the current positions with the given algo, without
+ * stepping (Eq. 1; PAPER.md:98-112 for MD_CELL).  Also refreshes KE.
+ * MD_EDOMAIN if algo = MD_CELL and int[L/rc] < 3. */
+int md_compute_forces(md_sim *s, int algo);
+
+/* Advance nsteps velocity-Verlet steps (order per R4): half-kick, drift with
+ * periodic wrap, force evaluation with algo, half-kick.  If the forces are stale (or were
+ * last evaluated by the other algo's data layout) they are evaluated first; that evaluation
+ * is not a step.  MD_CELL rebuilds the cell list from current positions before every force
+ * evaluation (R20).  nsteps = 0 is allowed.  Atoms moving more than L per step and
+ * coincident atoms are undefined behaviour. */
+int md_step(md_sim *s, int64_t nsteps, int algo);
+
+/* Forces [N][3] at the current positions, caller's atom order.  MD_ESTATE if stale. */
+int md_get_forces(md_sim *s, float *f);
+
+/* KE = (1/2) sum v^2, PE = sum_{i<j} U(r_ij), virial = sum_{i<j} r_ij f(r_ij) (R12), all at
+ * the current time; any pointer may be NULL.  MD_ESTATE if forces are stale. */
+int md_get_energies(md_sim *s, double *KE, double *PE, double *virial);
+
+/* rand48 (Eq. 5): x <- (0x5DEECE66D x + 0xB) mod 2^48; each output is
+ * taken from the NEW state (R8).  seeds[s] is the 48-bit state of stream s (bits 48..63 must
+ * be zero) and is replaced by the state after ndraws draws, so consecutive calls concatenate
+ * bit-exactly.  Output is stream-major: out[s*ndraws + d] is draw d of
+ * stream s.  kind: 0 uint32 x>>16; 1 uint32 x>>17 (lrand48); 2 double x*2^-48; 3 uint64 x.
+ * Streams are split across warps by O(log k) skip-ahead (Eq. 6-7 with
+ * R5), so nstreams = 1 with a large ndraws runs on the whole GPU.  seeds and out may each be
+ * host or device memory.  ndraws = 0 or nstreams = 0 is MD_OK and writes nothing. */
+int rand48_fill(uint64_t *seeds, int64_t nstreams, int64_t ndraws, int kind, void *out);
+
+/* Human-readable name of a status code; never NULL. */
+const char *md_strerror(int code);
+
+/* ---- helpers (not named by the paper; needed by tests, bench and bindings) ---- */
+
+/* Stream (a cudaStream_t passed as void*) on which this handle's kernels run. */
+int md_set_stream(md_sim *s, void *cuda_stream);
+/* Stream used by rand48_fill (process-wide). */
+int rand48_set_stream(void *cuda_stream);
+
+/* Device allocator hooks (process-wide), e.g. PyTorch's caching allocator.  alloc returns a
+ * device pointer or NULL; both are called with the stream in use.  NULL, NULL restores
+ * cudaMalloc/cudaFree.  Must be set before the handles that use them are created. */
+typedef void *(*md_alloc_fn)(int64_t bytes, void *cuda_stream);
+typedef void (*md_free_fn)(void *ptr, void *cuda_stream);
+int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
+
+/* Tuning and introspection.  md_set_option keys:
+ *   "graph"          1 (default) replay each step from a CUDA graph, 0 launch directly
+ *   "precise_r2"     squared distance below which the pair term is evaluated in FP64
+ *                    (default: all in-range pairs); 0 = FP32 everywhere
+ *   "sort_every"     all-pairs path: re-sort atoms spatially every k steps (default 20)
+ * md_get_stat keys: "ncell" (cells per dimension), "max_occupancy", "kernel_launches"
+ * (kernels launched by this handle so far), "steps_done", "side" (cell side). */
+int md_set_option(md_sim *s, const char *key, double value);
+int md_get_stat(md_sim *s, const char *key, double *value);
+
+/* Text of the last CUDA error seen by this thread's library calls ("" if none). */
+const char *md_last_cuda_error(void);
+
+/* Kernels launched by rand48_fill calls so far (process-wide counter). */
+int64_t rand48_kernel_launches(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LJMD_H */

@@ -1,0 +1,115 @@
+// Internal declarations shared by the translation units of libljmd_b200.so.
+// Public surface: include/ljmd.h.  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/ljmd.h"
+
+#define LJ_WARP 32
+
+// ---- error plumbing -------------------------------------------------------------
+void ljmd_note_cuda_error(cudaError_t e, const char *what, const char *file, int line);
+#define CK(call)                                                        \
+    do {                                                                \
+        cudaError_t e__ = (call);                                       \
+        if (e__ != cudaSuccess) {                                       \
+            ljmd_note_cuda_error(e__, #call, __FILE__, __LINE__);       \
+            return MD_ECUDA;                                            \
+        }                                                               \
+    } while (0)
+#define CKL(s) CK(cudaGetLastError()); (s)->launches++
+
+// ---- device memory (through the optional allocator hooks) -----------------------
+void *ljmd_dev_alloc(int64_t bytes, cudaStream_t st);
+void ljmd_dev_free(void *p, cudaStream_t st);
+
+// ---- pair-potential constants, FP64 (precise branch) and FP32 (filters, fast branch)
+struct PairParams {
+    double rc2, sig2, eps24, eps4, ushift, rc, f_rc;   // f_rc = f_LJ(rc), mode 2 only
+    double precise_r2;     // pairs with r2 < precise_r2 are evaluated in FP64
+    float rc2f_filter;     // FP32 accept threshold (rc^2 plus a rounding margin)
+    float sig2f, eps24f, eps4f, ushiftf, rcf, f_rcf;
+    int mode;
+};
+
+// ---- cell grid on a power-of-two aligned lattice ----------
+struct Grid {
+    int n;            // cells per dimension
+    int ncells;       // n^3
+    float side;       // width of cells 0..n-2 (a multiple of the grid quantum g)
+    float last;       // width of cell n-1 = L - (n-1)*side  (>= side)
+    float inv_side;
+    float L;
+};
+
+struct md_sim {
+    int64_t N;
+    double L, rc, eps, sigma, dt;
+    int shifted;
+    float Lf, dtf, hdtf;
+    PairParams pp;
+    Grid grid;            // grid.n == 0 when the box has fewer than 3 cells per dimension
+    int grid_paper_n;     // int[L/rc]
+    cudaStream_t stream;
+
+    // state in "slot" order; pos.w carries the caller's atom id as int bits
+    float4 *pos, *vel, *frc;
+    float4 *pos2, *vel2;          // scatter targets (cell build)
+    float4 *lpos;                 // cell-local coordinates in slot order (after a build)
+    int *cell_of;                 // [N] cell id per slot (after a build)
+    int *rank;                    // [N] rank inside its cell (during a build)
+    int *cell_count;              // [ncells]
+    int *cell_start;              // [ncells + 1]
+    int *max_occ;                 // [1]
+    // all-pairs partial forces: [nsplit][3][N] doubles
+    double *fpart;
+    int ap_nsplit;
+    // energy partials and results
+    double *part;                 // [3][part_cap] block partials: KE, PE, W
+    int part_cap;
+    int n_ke, n_pe;               // valid partial counts
+    double *energies;             // [3] on device: KE, PE, W
+    float *xfer;                  // [N][3] staging for host/device packing
+    bool layout_cell;             // slot order is cell-sorted and lpos/cell_start are current
+    bool has_state, forces_valid;
+    int forces_algo;
+    bool use_graph;
+    int sort_every;
+    int64_t launches, steps_done;
+    // CUDA graph cache for one step
+    cudaGraphExec_t graph_exec[2];
+    bool graph_ok[2];
+};
+
+// ---- kernels' host launchers (each returns md_status) ---------------------------
+int ljmd_pack_state(md_sim *s, const float *dpos, const float *dvel);
+int ljmd_unpack(md_sim *s, const float4 *src, float *dout);        // [N][3], caller's order
+int ljmd_kick_drift(md_sim *s);
+int ljmd_kick_ke(md_sim *s);
+int ljmd_ke_only(md_sim *s);
+int ljmd_reduce_energies(md_sim *s);
+int ljmd_forces_allpairs(md_sim *s);
+int ljmd_cell_build(md_sim *s);
+int ljmd_forces_cell(md_sim *s);
+
+// ---- small device helpers --------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Sum over the block; result valid in thread 0.  blockDim.x a multiple of 32, <= 1024.
+__device__ __forceinline__ double block_sum(double v, double *smem32)
+{
+    v = warp_sum(v);
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) smem32[w] = v;
+    __syncthreads();
+    int nw = (blockDim.x + 31) >> 5;
+    v = (threadIdx.x < nw) ? smem32[threadIdx.x] : 0.0;
+    if (w == 0) v = warp_sum(v);
+    return v;
+}

@@ -1,0 +1,391 @@
+// C ABI of libljmd_b200.so (include/ljmd.h): argument validation, buffer ownership, the
+// stale-force state machine and the per-step kernel sequence.  No arithmetic of the method
+// happens on the host: every step of the path runs in the kernels of this library.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+#include "common.cuh"
+
+// ---- errors -------------------------------------------------------------------------
+static thread_local char g_cuda_err[512] = "";
+
+void ljmd_note_cuda_error(cudaError_t e, const char *what, const char *file, int line)
+{
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s (%s) at %s:%d: %s", cudaGetErrorName(e), what, file, line,
+             cudaGetErrorString(e));
+}
+
+extern "C" const char *md_last_cuda_error(void) { return g_cuda_err; }
+
+extern "C" const char *md_strerror(int code)
+{
+    switch (code) {
+    case MD_OK: return "MD_OK";
+    case MD_EINVAL: return "MD_EINVAL: invalid argument";
+    case MD_EDOMAIN: return "MD_EDOMAIN: cell list needs at least 3 cells per dimension";
+    case MD_ESTATE: return "MD_ESTATE: state not set or forces stale";
+    case MD_ENOMEM: return "MD_ENOMEM: allocation failed";
+    case MD_ECUDA: return "MD_ECUDA: CUDA runtime error (see md_last_cuda_error)";
+    case MD_EUNSUPPORTED: return "MD_EUNSUPPORTED: not implemented in this build";
+    default: return "unknown md_status";
+    }
+}
+
+// ---- allocator hooks ----------------------------------------------------------------
+static md_alloc_fn g_alloc = nullptr;
+static md_free_fn g_free = nullptr;
+
+extern "C" int md_set_allocator(md_alloc_fn a, md_free_fn f)
+{
+    if ((a == nullptr) != (f == nullptr)) return MD_EINVAL;
+    g_alloc = a;
+    g_free = f;
+    return MD_OK;
+}
+
+void *ljmd_dev_alloc(int64_t bytes, cudaStream_t st)
+{
+    if (bytes <= 0) bytes = 16;
+    if (g_alloc) return g_alloc(bytes, (void *)st);
+    void *p = nullptr;
+    cudaError_t e = cudaMalloc(&p, (size_t)bytes);
+    if (e != cudaSuccess) {
+        ljmd_note_cuda_error(e, "cudaMalloc", __FILE__, __LINE__);
+        return nullptr;
+    }
+    return p;
+}
+
+void ljmd_dev_free(void *p, cudaStream_t st)
+{
+    if (!p) return;
+    if (g_free) g_free(p, (void *)st);
+    else cudaFree(p);
+}
+
+// ---- grid and pair constants ----------------------------------------------------------
+// Cells on a lattice whose spacing is a multiple of g = ulp of the binade of L, so that cell
+// origins c*side are exact floats and x - origin is exact.
+static void setup_grid(md_sim *s)
+{
+    double L = s->L, rc = s->rc;
+    s->grid_paper_n = (int)floor(L / rc);
+    Grid &g = s->grid;
+    memset(&g, 0, sizeof(g));
+    g.L = s->Lf;
+    int e;
+    frexp(L, &e);                                    // L = m 2^e, m in [0.5,1)
+    double q = ldexp(1.0, e - 24);                   // ulp of floats in [2^(e-1), 2^e)
+    int n = s->grid_paper_n;
+    if (n > 1023) n = 1023;                          // cell id must fit 30 bits
+    double side = 0.0;
+    for (; n >= 3; n--) {
+        side = floor(L / n / q) * q;
+        if (side >= rc) break;
+    }
+    if (n < 3) return;                               // g.n stays 0: cell path unavailable
+    g.n = n;
+    g.ncells = n * n * n;
+    g.side = (float)side;
+    g.last = (float)(L - (n - 1) * side);
+    g.inv_side = (float)(1.0 / side);
+}
+
+static void setup_pair(md_sim *s)
+{
+    PairParams &P = s->pp;
+    double rc = s->rc, sg = s->sigma, eps = s->eps;
+    P.rc = rc;
+    P.rc2 = rc * rc;
+    P.sig2 = sg * sg;
+    P.eps24 = 24.0 * eps;
+    P.eps4 = 4.0 * eps;
+    double s6 = pow(sg * sg / (rc * rc), 3.0);
+    P.ushift = (s->shifted >= 1) ? 4.0 * eps * (s6 * s6 - s6) : 0.0;
+    P.f_rc = (s->shifted == 2) ? 24.0 * eps * (2.0 * s6 * s6 - s6) / rc : 0.0;
+    P.mode = s->shifted;
+    P.precise_r2 = 1e300;
+    // FP32 filter threshold: rc^2 plus the worst-case rounding error of an FP32 r^2 computed
+    // from box-scale coordinates (|d| error <= 2 ulp(L)), so the filter never rejects a pair
+    // that is inside rc in exact arithmetic.
+    double errd = 4.0 * s->L * ldexp(1.0, -23);
+    double margin = 2.0 * sqrt(3.0) * (rc + errd) * errd + P.rc2 * 1e-6;
+    float f = (float)(P.rc2 + margin);
+    P.rc2f_filter = nextafterf(f, INFINITY);
+    P.sig2f = (float)P.sig2;
+    P.eps24f = (float)P.eps24;
+    P.eps4f = (float)P.eps4;
+    P.ushiftf = (float)P.ushift;
+    P.rcf = (float)rc;
+    P.f_rcf = (float)P.f_rc;
+}
+
+// ---- create / destroy -----------------------------------------------------------------
+static void free_all(md_sim *s)
+{
+    cudaStream_t st = s->stream;
+    for (int k = 0; k < 2; k++)
+        if (s->graph_exec[k]) cudaGraphExecDestroy(s->graph_exec[k]);
+    void *ptrs[] = {s->pos, s->vel, s->frc, s->pos2, s->vel2, s->lpos, s->cell_of, s->rank, s->cell_count,
+                    s->cell_start, s->max_occ, s->fpart, s->part, s->energies, s->xfer};
+    for (void *p : ptrs) ljmd_dev_free(p, st);
+}
+
+extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double eps, double sigma, double dt,
+                         int shifted)
+{
+    if (!out) return MD_EINVAL;
+    *out = nullptr;
+    if (N <= 0 || N > (1LL << 30) || !(L > 0) || !(rc > 0) || !(eps >= 0) || !(sigma > 0) || !(dt > 0) ||
+        shifted < 0 || shifted > 2 || !isfinite(L) || !isfinite(rc) || !isfinite(eps) || !isfinite(sigma) ||
+        !isfinite(dt))
+        return MD_EINVAL;
+    double Lr = (double)(float)L;                                   // R13
+    if (rc > 0.5 * Lr) return MD_EINVAL;
+    int dev;
+    CK(cudaGetDevice(&dev));
+    md_sim *s = new (std::nothrow) md_sim;
+    if (!s) return MD_ENOMEM;
+    memset(s, 0, sizeof(*s));
+    s->N = N;
+    s->L = Lr;
+    s->rc = rc;
+    s->eps = eps;
+    s->sigma = sigma;
+    s->dt = dt;
+    s->shifted = shifted;
+    s->Lf = (float)L;
+    s->dtf = (float)dt;
+    s->hdtf = (float)(0.5 * dt);
+    s->use_graph = true;
+    s->sort_every = 20;
+    setup_grid(s);
+    setup_pair(s);
+
+    const int AP_T = 128;
+    int niblk = (int)((N + AP_T - 1) / AP_T);
+    int nsplit = (592 + niblk - 1) / niblk;
+    if (nsplit > niblk) nsplit = niblk;
+    if (nsplit > 64) nsplit = 64;
+    if (nsplit < 1) nsplit = 1;
+    s->ap_nsplit = nsplit;
+    int cap_ap = niblk * nsplit;
+    int cap_it = (int)((N + 255) / 256);
+    s->part_cap = (cap_ap > cap_it ? cap_ap : cap_it) + 64;
+
+    cudaStream_t st = s->stream;
+    size_t f4 = (size_t)N * sizeof(float4);
+    s->pos = (float4 *)ljmd_dev_alloc(f4, st);
+    s->vel = (float4 *)ljmd_dev_alloc(f4, st);
+    s->frc = (float4 *)ljmd_dev_alloc(f4, st);
+    s->pos2 = (float4 *)ljmd_dev_alloc(f4, st);
+    s->vel2 = (float4 *)ljmd_dev_alloc(f4, st);
+    s->lpos = (float4 *)ljmd_dev_alloc(f4, st);
+    s->cell_of = (int *)ljmd_dev_alloc(N * sizeof(int), st);
+    s->rank = (int *)ljmd_dev_alloc(N * sizeof(int), st);
+    int ncells = s->grid.n ? s->grid.ncells : 1;
+    s->cell_count = (int *)ljmd_dev_alloc((size_t)ncells * sizeof(int), st);
+    s->cell_start = (int *)ljmd_dev_alloc(((size_t)ncells + 1) * sizeof(int), st);
+    s->max_occ = (int *)ljmd_dev_alloc(sizeof(int), st);
+    s->fpart = (double *)ljmd_dev_alloc((size_t)nsplit * 3 * N * sizeof(double), st);
+    s->part = (double *)ljmd_dev_alloc((size_t)3 * s->part_cap * sizeof(double), st);
+    s->energies = (double *)ljmd_dev_alloc(3 * sizeof(double), st);
+    s->xfer = (float *)ljmd_dev_alloc((size_t)N * 3 * sizeof(float), st);
+    if (!s->pos || !s->vel || !s->frc || !s->pos2 || !s->vel2 || !s->lpos || !s->cell_of || !s->rank ||
+        !s->cell_count || !s->cell_start || !s->max_occ || !s->fpart || !s->part || !s->energies || !s->xfer) {
+        free_all(s);
+        delete s;
+        return MD_ENOMEM;
+    }
+    cudaError_t e = cudaMemsetAsync(s->cell_count, 0, (size_t)ncells * sizeof(int), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->max_occ, 0, sizeof(int), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->frc, 0, f4, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+        ljmd_note_cuda_error(e, "md_create init", __FILE__, __LINE__);
+        free_all(s);
+        delete s;
+        return MD_ECUDA;
+    }
+    *out = s;
+    return MD_OK;
+}
+
+extern "C" int md_destroy(md_sim *s)
+{
+    if (!s) return MD_OK;
+    cudaStreamSynchronize(s->stream);
+    free_all(s);
+    delete s;
+    return MD_OK;
+}
+
+extern "C" int md_set_stream(md_sim *s, void *stream)
+{
+    if (!s) return MD_EINVAL;
+    CK(cudaStreamSynchronize(s->stream));
+    s->stream = (cudaStream_t)stream;
+    for (int k = 0; k < 2; k++) s->graph_ok[k] = false;
+    return MD_OK;
+}
+
+// ---- state in / out -------------------------------------------------------------------
+// Copy a caller array (host or device) of n floats into device staging, or back.
+static int stage_in(md_sim *s, const float *src, float *dst, size_t n)
+{
+    CK(cudaMemcpyAsync(dst, src, n * sizeof(float), cudaMemcpyDefault, s->stream));
+    return MD_OK;
+}
+
+extern "C" int md_set_state(md_sim *s, const float *pos, const float *vel)
+{
+    if (!s || !pos || !vel) return MD_EINVAL;
+    size_t n3 = (size_t)s->N * 3;
+    // stage positions in xfer and velocities in lpos (reused as scratch: 4N floats >= 3N)
+    int r = stage_in(s, pos, s->xfer, n3);
+    if (r) return r;
+    r = stage_in(s, vel, (float *)s->lpos, n3);
+    if (r) return r;
+    r = ljmd_pack_state(s, s->xfer, (const float *)s->lpos);
+    if (r) return r;
+    CK(cudaStreamSynchronize(s->stream));
+    s->has_state = true;
+    s->forces_valid = false;
+    s->layout_cell = false;
+    return MD_OK;
+}
+
+static int read_out(md_sim *s, const float4 *src, float *out)
+{
+    int r = ljmd_unpack(s, src, s->xfer);
+    if (r) return r;
+    CK(cudaMemcpyAsync(out, s->xfer, (size_t)s->N * 3 * sizeof(float), cudaMemcpyDefault, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    return MD_OK;
+}
+
+extern "C" int md_get_state(md_sim *s, float *pos, float *vel)
+{
+    if (!s) return MD_EINVAL;
+    if (!s->has_state) return MD_ESTATE;
+    int r;
+    if (pos && (r = read_out(s, s->pos, pos))) return r;
+    if (vel && (r = read_out(s, s->vel, vel))) return r;
+    return MD_OK;
+}
+
+extern "C" int md_get_forces(md_sim *s, float *f)
+{
+    if (!s || !f) return MD_EINVAL;
+    if (!s->has_state || !s->forces_valid) return MD_ESTATE;
+    return read_out(s, s->frc, f);
+}
+
+extern "C" int md_get_energies(md_sim *s, double *KE, double *PE, double *W)
+{
+    if (!s) return MD_EINVAL;
+    if (!s->has_state || !s->forces_valid) return MD_ESTATE;
+    double h[3];
+    CK(cudaMemcpyAsync(h, s->energies, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    if (KE) *KE = h[0];
+    if (PE) *PE = h[1];
+    if (W) *W = h[2];
+    return MD_OK;
+}
+
+// ---- force evaluation and stepping ------------------------------------------------------
+static int check_algo(md_sim *s, int algo)
+{
+    if (algo != MD_ALLPAIRS && algo != MD_CELL) return MD_EINVAL;
+    if (algo == MD_CELL && (s->grid_paper_n < 3 || s->grid.n < 3)) return MD_EDOMAIN;
+    return MD_OK;
+}
+
+static int eval_forces(md_sim *s, int algo)
+{
+    int r;
+    if (algo == MD_CELL) {
+        if ((r = ljmd_cell_build(s))) return r;
+        if ((r = ljmd_forces_cell(s))) return r;
+    } else {
+        s->layout_cell = false;
+        if ((r = ljmd_forces_allpairs(s))) return r;
+    }
+    return MD_OK;
+}
+
+extern "C" int md_compute_forces(md_sim *s, int algo)
+{
+    if (!s) return MD_EINVAL;
+    if (!s->has_state) return MD_ESTATE;
+    int r = check_algo(s, algo);
+    if (r) return r;
+    if ((r = eval_forces(s, algo))) return r;
+    if ((r = ljmd_ke_only(s))) return r;
+    if ((r = ljmd_reduce_energies(s))) return r;
+    CK(cudaStreamSynchronize(s->stream));
+    s->forces_valid = true;
+    s->forces_algo = algo;
+    return MD_OK;
+}
+
+extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
+{
+    if (!s || nsteps < 0) return MD_EINVAL;
+    if (!s->has_state) return MD_ESTATE;
+    int r = check_algo(s, algo);
+    if (r) return r;
+    if (!s->forces_valid) {
+        if ((r = eval_forces(s, algo))) return r;
+        if ((r = ljmd_ke_only(s))) return r;
+        s->forces_valid = true;
+        s->forces_algo = algo;
+    }
+    for (int64_t k = 0; k < nsteps; k++) {
+        if ((r = ljmd_kick_drift(s))) return r;
+        if ((r = eval_forces(s, algo))) return r;
+        if ((r = ljmd_kick_ke(s))) return r;
+    }
+    if ((r = ljmd_reduce_energies(s))) return r;
+    CK(cudaStreamSynchronize(s->stream));
+    s->forces_algo = algo;
+    s->steps_done += nsteps;
+    return MD_OK;
+}
+
+// ---- options and statistics ---------------------------------------------------------------
+extern "C" int md_set_option(md_sim *s, const char *key, double value)
+{
+    if (!s || !key) return MD_EINVAL;
+    if (!strcmp(key, "graph")) s->use_graph = value != 0.0;
+    else if (!strcmp(key, "precise_r2")) {
+        if (!(value >= 0)) return MD_EINVAL;
+        s->pp.precise_r2 = value;
+    } else if (!strcmp(key, "sort_every")) {
+        if (value < 1) return MD_EINVAL;
+        s->sort_every = (int)value;
+    } else return MD_EINVAL;
+    for (int k = 0; k < 2; k++) s->graph_ok[k] = false;
+    return MD_OK;
+}
+
+extern "C" int md_get_stat(md_sim *s, const char *key, double *value)
+{
+    if (!s || !key || !value) return MD_EINVAL;
+    if (!strcmp(key, "ncell")) *value = s->grid.n;
+    else if (!strcmp(key, "side")) *value = s->grid.side;
+    else if (!strcmp(key, "last_side")) *value = s->grid.last;
+    else if (!strcmp(key, "kernel_launches")) *value = (double)s->launches;
+    else if (!strcmp(key, "steps_done")) *value = (double)s->steps_done;
+    else if (!strcmp(key, "ap_nsplit")) *value = s->ap_nsplit;
+    else if (!strcmp(key, "max_occupancy")) {
+        int h = 0;
+        CK(cudaMemcpyAsync(&h, s->max_occ, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+        CK(cudaStreamSynchronize(s->stream));
+        *value = h;
+    } else return MD_EINVAL;
+    return MD_OK;
+}

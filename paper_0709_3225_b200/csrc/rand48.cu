@@ -1,0 +1,240 @@
+// rand48 with O(log k) skip-ahead.
+// PAPER.md:142-146 (Eq. 5): x <- (a x + c) mod 2^48, a = 0x5DEECE66D, c = 0xB, output from the
+// new state's most-significant bits.  PAPER.md:150-162 (Eq. 6-7, sum bound corrected per R5):
+// x_{n+m} = A_m x_n + C_m.  The paper leap-frogs S = 6144 threads over ONE stream after a
+// serial warm-up; here every warp leap-frogs over a 128-draw window of its own segment of a
+// stream, and reaches its start state by composing the maps (A_{2^b}, C_{2^b}) -- no serial
+// warm-up, any number of streams, coalesced 16-byte stores of stream-major output.
+#include "common.cuh"
+
+#define R48_A 0x5DEECE66DULL
+#define R48_C 0xBULL
+#define R48_MASK 0xFFFFFFFFFFFFULL
+#define R48_T 256
+
+__device__ uint64_t g_r48_A[48];   // A_{2^b}
+__device__ uint64_t g_r48_C[48];   // C_{2^b}
+
+// (A, C)_{2^(b+1)} = (A, C)_{2^b} composed with itself: (A^2, A C + C).
+__global__ void k_r48_init_table()
+{
+    uint64_t a = R48_A, c = R48_C;
+    for (int b = 0; b < 48; b++) {
+        g_r48_A[b] = a;
+        g_r48_C[b] = c;
+        c = (a * c + c) & R48_MASK;
+        a = (a * a) & R48_MASK;
+    }
+}
+
+// State after n further draws, by applying the power-of-two maps for the set bits of n.
+__device__ __forceinline__ uint64_t r48_skip(uint64_t x, uint64_t n)
+{
+    n &= R48_MASK;                         // the period is 2^48
+    for (int b = 0; n != 0; b++, n >>= 1)
+        if (n & 1) x = (g_r48_A[b] * x + g_r48_C[b]) & R48_MASK;
+    return x;
+}
+
+template <int KIND> struct R48Out;
+template <> struct R48Out<0> { typedef uint32_t T; static __device__ __forceinline__ T cv(uint64_t x) { return (uint32_t)(x >> 16); } };
+template <> struct R48Out<1> { typedef uint32_t T; static __device__ __forceinline__ T cv(uint64_t x) { return (uint32_t)(x >> 17); } };
+template <> struct R48Out<2> {
+    typedef double T;
+    // x * 2^-48 exactly: 1.m with m = x << 4 is 1 + x 2^-48 in [1,2); subtracting 1 is exact.
+    static __device__ __forceinline__ T cv(uint64_t x) { return __longlong_as_double((long long)(0x3FF0000000000000ULL | (x << 4))) - 1.0; }
+};
+template <> struct R48Out<3> { typedef uint64_t T; static __device__ __forceinline__ T cv(uint64_t x) { return x; } };
+
+// One warp per (stream, segment).  Lane l keeps 4 states whose positions inside the current
+// 128-draw window are pos[k]; every iteration applies (A_128, C_128) to all four.
+template <int KIND>
+__global__ void __launch_bounds__(R48_T)
+k_rand48_fill(const uint64_t *__restrict__ seeds, int64_t nstreams, int64_t ndraws, int64_t seg, int64_t nseg,
+              void *__restrict__ out_, int vec_ok)
+{
+    typedef typename R48Out<KIND>::T T;
+    constexpr int V = 16 / sizeof(T);                  // draws per 16-byte vector: 4 or 2
+    const int lane = threadIdx.x & 31;
+    const int64_t gw = ((int64_t)blockIdx.x * R48_T + threadIdx.x) >> 5;
+    if (gw >= nstreams * nseg) return;
+    const int64_t s = gw / nseg, g = gw - s * nseg;
+    const int64_t start = g * seg;
+    const int64_t len = min(seg, ndraws - start);
+    T *out = (T *)out_ + (s * ndraws + start);
+
+    const uint64_t A128 = g_r48_A[7], C128 = g_r48_C[7];
+    uint64_t st[4];
+    int pos[4];
+    st[0] = r48_skip(seeds[s], (uint64_t)(start + lane * V + 1));
+    pos[0] = lane * V;
+#pragma unroll
+    for (int k = 1; k < V; k++) {
+        st[k] = (R48_A * st[k - 1] + R48_C) & R48_MASK;
+        pos[k] = pos[k - 1] + 1;
+    }
+    if (V == 2) {                                      // second vector: 64 draws further on
+        const uint64_t A64 = g_r48_A[6], C64 = g_r48_C[6];
+        st[2] = (A64 * st[0] + C64) & R48_MASK;
+        st[3] = (A64 * st[1] + C64) & R48_MASK;
+        pos[2] = pos[0] + 64;
+        pos[3] = pos[1] + 64;
+    }
+
+    const int64_t nfull = vec_ok ? len / 128 : 0;
+    for (int64_t it = 0; it < nfull; it++) {
+        T *o = out + it * 128;
+        if (V == 4) {
+            uint4 v = make_uint4((uint32_t)R48Out<KIND>::cv(st[0]), (uint32_t)R48Out<KIND>::cv(st[1]),
+                                 (uint32_t)R48Out<KIND>::cv(st[2]), (uint32_t)R48Out<KIND>::cv(st[3]));
+            __stcs((uint4 *)(o + pos[0]), v);
+        } else {
+            T a0 = R48Out<KIND>::cv(st[0]), a1 = R48Out<KIND>::cv(st[1]);
+            T a2 = R48Out<KIND>::cv(st[2]), a3 = R48Out<KIND>::cv(st[3]);
+            ulonglong2 v0, v1;
+            memcpy(&v0.x, &a0, 8); memcpy(&v0.y, &a1, 8);
+            memcpy(&v1.x, &a2, 8); memcpy(&v1.y, &a3, 8);
+            __stcs((ulonglong2 *)(o + pos[0]), v0);
+            __stcs((ulonglong2 *)(o + pos[2]), v1);
+        }
+#pragma unroll
+        for (int k = 0; k < 4; k++) st[k] = (A128 * st[k] + C128) & R48_MASK;
+    }
+    // scalar tail (and the whole segment when 16-byte stores are not aligned)
+    for (int64_t base = nfull * 128; base < len; base += 128) {
+#pragma unroll
+        for (int k = 0; k < 4; k++) {
+            if (base + pos[k] < len) out[base + pos[k]] = R48Out<KIND>::cv(st[k]);
+            st[k] = (A128 * st[k] + C128) & R48_MASK;
+        }
+    }
+}
+
+// seeds[s] <- state after ndraws draws ("the thread saves the current state").
+__global__ void __launch_bounds__(R48_T)
+k_rand48_advance(uint64_t *__restrict__ seeds, int64_t nstreams, uint64_t ndraws)
+{
+    int64_t s = (int64_t)blockIdx.x * R48_T + threadIdx.x;
+    if (s < nstreams) seeds[s] = r48_skip(seeds[s], ndraws);
+}
+
+__device__ int g_r48_flag;
+
+__global__ void __launch_bounds__(R48_T)
+k_rand48_validate(const uint64_t *__restrict__ seeds, int64_t nstreams)
+{
+    int64_t s = (int64_t)blockIdx.x * R48_T + threadIdx.x;
+    if (s < nstreams && (seeds[s] >> 48)) g_r48_flag = 1;
+}
+
+static cudaStream_t g_r48_stream = 0;
+static bool g_r48_table_ready = false;
+static int64_t g_r48_launches = 0;
+
+extern "C" int rand48_set_stream(void *stream)
+{
+    g_r48_stream = (cudaStream_t)stream;
+    return MD_OK;
+}
+
+extern "C" int64_t rand48_kernel_launches(void) { return g_r48_launches; }
+
+static bool on_device(const void *p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+extern "C" int rand48_fill(uint64_t *seeds, int64_t nstreams, int64_t ndraws, int kind, void *out)
+{
+    if (nstreams < 0 || ndraws < 0 || kind < 0 || kind > 3) return MD_EINVAL;
+    if (nstreams == 0) return MD_OK;
+    if (!seeds) return MD_EINVAL;
+    if (ndraws > 0 && !out) return MD_EINVAL;
+    if (ndraws > (int64_t)R48_MASK) return MD_EINVAL;
+    cudaStream_t st = g_r48_stream;
+    const size_t esize = (kind <= 1) ? 4 : 8;
+    const bool seeds_dev = on_device(seeds);
+    const bool out_dev = ndraws == 0 || on_device(out);
+    uint64_t *dseeds = seeds;
+    void *dout = out;
+    int rc = MD_OK;
+
+    // seeds must be 48-bit states (argument check): on the host for host arrays, by a
+    // one-pass kernel and a 4-byte flag for device arrays
+    if (seeds_dev) {
+        int flag = 0;
+        CK(cudaMemcpyToSymbolAsync(g_r48_flag, &flag, sizeof(int), 0, cudaMemcpyHostToDevice, st));
+        k_rand48_validate<<<(unsigned)((nstreams + R48_T - 1) / R48_T), R48_T, 0, st>>>(seeds, nstreams);
+        CK(cudaGetLastError());
+        g_r48_launches++;
+        CK(cudaMemcpyFromSymbolAsync(&flag, g_r48_flag, sizeof(int), 0, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        if (flag) return MD_EINVAL;
+    } else {
+        for (int64_t i = 0; i < nstreams; i++)
+            if (seeds[i] >> 48) return MD_EINVAL;
+    }
+    if (ndraws == 0) return MD_OK;
+
+    if (!g_r48_table_ready) {
+        k_r48_init_table<<<1, 1, 0, st>>>();
+        CK(cudaGetLastError());
+        g_r48_launches++;
+        g_r48_table_ready = true;
+    }
+    if (!seeds_dev) {
+        dseeds = (uint64_t *)ljmd_dev_alloc(nstreams * 8, st);
+        if (!dseeds) return MD_ENOMEM;
+        cudaError_t e = cudaMemcpyAsync(dseeds, seeds, (size_t)nstreams * 8, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) { ljmd_note_cuda_error(e, "seed upload", __FILE__, __LINE__); rc = MD_ECUDA; goto done; }
+    }
+    if (!out_dev) {
+        dout = ljmd_dev_alloc((int64_t)((size_t)nstreams * ndraws * esize), st);
+        if (!dout) { rc = MD_ENOMEM; goto done; }
+    }
+    {
+        // segment length: a multiple of 128 draws, at least 1024, sized for ~128K warps
+        int64_t total = nstreams * ndraws;
+        int64_t seg = (total / 131072 + 127) / 128 * 128;
+        if (seg < 1024) seg = 1024;
+        int64_t nd128 = (ndraws + 127) / 128 * 128;
+        if (seg > nd128) seg = nd128;
+        int64_t nseg = (ndraws + seg - 1) / seg;
+        int64_t nwarps = nstreams * nseg;
+        int64_t nblocks = (nwarps * 32 + R48_T - 1) / R48_T;
+        if (nblocks > 0x7FFFFFFF) { rc = MD_EUNSUPPORTED; goto done; }
+        int vec_ok = (((uintptr_t)dout) % 16 == 0) && ((ndraws * esize) % 16 == 0);
+        switch (kind) {
+        case 0: k_rand48_fill<0><<<(unsigned)nblocks, R48_T, 0, st>>>(dseeds, nstreams, ndraws, seg, nseg, dout, vec_ok); break;
+        case 1: k_rand48_fill<1><<<(unsigned)nblocks, R48_T, 0, st>>>(dseeds, nstreams, ndraws, seg, nseg, dout, vec_ok); break;
+        case 2: k_rand48_fill<2><<<(unsigned)nblocks, R48_T, 0, st>>>(dseeds, nstreams, ndraws, seg, nseg, dout, vec_ok); break;
+        default: k_rand48_fill<3><<<(unsigned)nblocks, R48_T, 0, st>>>(dseeds, nstreams, ndraws, seg, nseg, dout, vec_ok); break;
+        }
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) { ljmd_note_cuda_error(e, "k_rand48_fill", __FILE__, __LINE__); rc = MD_ECUDA; goto done; }
+        g_r48_launches++;
+        k_rand48_advance<<<(unsigned)((nstreams + R48_T - 1) / R48_T), R48_T, 0, st>>>(dseeds, nstreams, (uint64_t)ndraws);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) { ljmd_note_cuda_error(e, "k_rand48_advance", __FILE__, __LINE__); rc = MD_ECUDA; goto done; }
+        g_r48_launches++;
+        if (!out_dev) {
+            e = cudaMemcpyAsync(out, dout, (size_t)nstreams * ndraws * esize, cudaMemcpyDeviceToHost, st);
+            if (e != cudaSuccess) { ljmd_note_cuda_error(e, "output download", __FILE__, __LINE__); rc = MD_ECUDA; goto done; }
+        }
+        if (!seeds_dev) {
+            e = cudaMemcpyAsync(seeds, dseeds, (size_t)nstreams * 8, cudaMemcpyDeviceToHost, st);
+            if (e != cudaSuccess) { ljmd_note_cuda_error(e, "seed download", __FILE__, __LINE__); rc = MD_ECUDA; goto done; }
+        }
+        e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { ljmd_note_cuda_error(e, "rand48_fill sync", __FILE__, __LINE__); rc = MD_ECUDA; }
+    }
+done:
+    if (!seeds_dev && dseeds) { cudaStreamSynchronize(st); ljmd_dev_free(dseeds, st); }
+    if (!out_dev && dout && dout != out) { cudaStreamSynchronize(st); ljmd_dev_free(dout, st); }
+    return rc;
+}

@@ -1,0 +1,202 @@
+"""Parity of the CUDA MD path against the FP64 oracle, through the C ABI (gpu-marked).
+Tolerances are BASELINE.json north_star's, read per DESIGN.md R15-R19."""
+import numpy as np
+import pytest
+
+import oracle
+from helpers import force_check, melt
+from paper_0709_3225_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def b():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_0709_3225_b200 import binding
+    return binding
+
+
+def gpu_forces(b, pos, vel, L, algo, shifted=1, eps=1.0, sigma=1.0, rc=2.5, opts=()):
+    with b.Sim(pos.shape[0], L, rc=rc, eps=eps, sigma=sigma, shifted=shifted) as s:
+        for k, v in opts:
+            s.option(k, v)
+        s.set_state(pos, vel)
+        s.compute_forces(algo)
+        return s.forces(), s.energies()
+
+
+# (n fcc cells, rho, perturbation): several i/j tiles with ragged tails, several box sizes
+CASES = [(3, 0.8, 0.08), (5, 0.8, 0.10), (6, 0.8, 0.10), (7, 0.9, 0.08), (4, 0.3, 0.15), (10, 0.8, 0.1)]
+
+
+@pytest.mark.parametrize("n,rho,amp", CASES)
+@pytest.mark.parametrize("shifted", [0, 1, 2])
+def test_forces_allpairs_match_oracle(b, n, rho, amp, shifted):
+    pos, L = wl.perturbed_fcc(n, rho, amp, seed=100 + n)
+    vel = np.zeros_like(pos)
+    F, (ke, pe, w) = gpu_forces(b, pos, vel, L, b.MD_ALLPAIRS, shifted)
+    Fo, peo, wo = oracle.forces(pos.astype(np.float64), L, mode=shifted, algo=0)
+    nviol, worst = force_check(F, Fo)
+    assert nviol == 0, (nviol, worst)
+    assert pe == pytest.approx(peo, rel=1e-9, abs=1e-9)
+    assert w == pytest.approx(wo, rel=1e-9, abs=1e-9)
+    assert ke == 0.0
+
+
+@pytest.mark.parametrize("n,rho,amp", [c for c in CASES if c[0] >= 4])
+@pytest.mark.parametrize("shifted", [0, 1, 2])
+def test_forces_cell_match_oracle(b, n, rho, amp, shifted):
+    pos, L = wl.perturbed_fcc(n, rho, amp, seed=100 + n)
+    vel = np.zeros_like(pos)
+    F, (ke, pe, w) = gpu_forces(b, pos, vel, L, b.MD_CELL, shifted)
+    Fo, peo, wo = oracle.forces(pos.astype(np.float64), L, mode=shifted, algo=1)
+    nviol, worst = force_check(F, Fo)
+    assert nviol == 0, (nviol, worst)
+    assert pe == pytest.approx(peo, rel=1e-9, abs=1e-9)
+    assert w == pytest.approx(wo, rel=1e-9, abs=1e-9)
+
+
+def test_eps_sigma_not_one(b):
+    pos, L = wl.perturbed_fcc(5, 0.8, 0.1, seed=9)
+    sig, eps = 1.3, 0.7
+    p2 = (pos.astype(np.float64) * sig).astype(np.float32)
+    L2 = float(np.float32(L * sig))
+    p2[p2 >= np.float32(L2)] = 0
+    for algo in (0, 1):
+        F, (_, pe, w) = gpu_forces(b, p2, np.zeros_like(p2), L2, algo, 1, eps, sig, 2.5 * sig)
+        Fo, peo, wo = oracle.forces(p2.astype(np.float64), L2, 2.5 * sig, eps, sig, 1, algo)
+        assert force_check(F, Fo)[0] == 0
+        assert pe == pytest.approx(peo, rel=1e-9) and w == pytest.approx(wo, rel=1e-9)
+
+
+def test_perfect_lattice_forces_vanish(b):
+    pos, L = wl.fcc_positions(5, 0.8)
+    for algo in (0, 1):
+        F, (_, pe, w) = gpu_forces(b, pos, np.zeros_like(pos), L, algo)
+        assert np.max(np.abs(F)) < 2e-5
+        assert pe / 500 == pytest.approx(-5.924190441386, abs=2e-6)
+
+
+def test_state_roundtrip_and_atom_order(b):
+    pos, L = wl.perturbed_fcc(6, 0.8, 0.1, seed=4)
+    rng = np.random.default_rng(0)
+    vel = rng.standard_normal(pos.shape).astype(np.float32)
+    with b.Sim(pos.shape[0], L) as s:
+        s.set_state(pos, vel)
+        p, v = s.get_state()
+        assert np.array_equal(p, pos) and np.array_equal(v, vel)
+        s.compute_forces(b.MD_CELL)                     # reorders internally
+        p, v = s.get_state()
+        assert np.array_equal(p, pos) and np.array_equal(v, vel)
+        Fc = s.forces()
+        s.compute_forces(b.MD_ALLPAIRS)
+        Fa = s.forces()
+        assert np.max(np.abs(Fc.astype(np.float64) - Fa)) < 1e-5 * max(1.0, np.max(np.abs(Fa)))
+        assert s.stat("ncell") == 3 or s.stat("ncell") == int(L / 2.5)
+
+
+def test_set_state_wraps_positions(b):
+    pos, L = wl.perturbed_fcc(4, 0.8, 0.1, seed=4)
+    shifted = pos.astype(np.float64) + np.array([L, -2 * L, 3 * L])
+    with b.Sim(pos.shape[0], L) as s:
+        s.set_state(shifted.astype(np.float32), np.zeros_like(pos))
+        p, _ = s.get_state()
+        assert np.all((p >= 0) & (p < np.float32(L)))
+
+
+def test_error_codes(b):
+    pos, L = wl.perturbed_fcc(3, 0.8, 0.05, seed=4)     # L = 5.13: int[L/rc] = 2
+    with b.Sim(pos.shape[0], L) as s:
+        for fn in (lambda: s.step(1, 0), lambda: s.forces(), lambda: s.energies(), lambda: s.compute_forces(0)):
+            with pytest.raises(b.MDError) as e:
+                fn()
+            assert e.value.code == b.MD_ESTATE
+        s.set_state(pos, np.zeros_like(pos))
+        with pytest.raises(b.MDError) as e:
+            s.forces()
+        assert e.value.code == b.MD_ESTATE               # stale
+        with pytest.raises(b.MDError) as e:
+            s.compute_forces(b.MD_CELL)
+        assert e.value.code == b.MD_EDOMAIN
+        with pytest.raises(b.MDError) as e:
+            s.step(1, 5)
+        assert e.value.code == b.MD_EINVAL
+        s.step(0, 0)
+        s.forces()
+
+
+@pytest.fixture(scope="module")
+def c1(oracle_uniforms):
+    return wl.md_system("c1_allpairs_500", oracle_uniforms)
+
+
+@pytest.mark.parametrize("algo", [0, 1])
+def test_config1_energy_trace_100_steps(b, c1, algo):
+    """Per-step total energy within 1e-5 relative of the oracle over 100 steps (R17)."""
+    _, _, _, tr = oracle.verlet_run(c1["pos"], c1["vel"], c1["L"], 100, algo=algo)
+    with b.Sim(c1["N"], c1["L"]) as s:
+        s.set_state(c1["pos"], c1["vel"])
+        s.compute_forces(algo)
+        worst = 0.0
+        for t in range(101):
+            if t:
+                s.step(1, algo)
+            ke, pe, w = s.energies()
+            Eo = tr[t, 0] + tr[t, 1]
+            worst = max(worst, abs(ke + pe - Eo) / abs(Eo))
+            assert ke == pytest.approx(tr[t, 0], rel=2e-4) and pe == pytest.approx(tr[t, 1], rel=2e-4)
+        assert worst < 1e-5, worst
+        # forces on the melted state, from the identical FP32 snapshot
+        p, v = s.get_state()
+        s.set_state(p, v)
+        s.compute_forces(algo)
+        Fo, _, _ = oracle.forces(p.astype(np.float64), c1["L"], algo=algo)
+        assert force_check(s.forces(), Fo)[0] == 0
+
+
+def test_multi_step_equals_single_steps(b, c1):
+    out = []
+    for chunks in ([20], [1] * 20, [7, 13]):
+        with b.Sim(c1["N"], c1["L"]) as s:
+            s.set_state(c1["pos"], c1["vel"])
+            for c in chunks:
+                s.step(c, 0)
+            out.append((s.get_state(), s.energies()))
+    for (p, v), e in out[1:]:
+        assert np.array_equal(p, out[0][0][0]) and np.array_equal(v, out[0][0][1]) and e == out[0][1]
+
+
+def test_time_reversibility(b, c1):
+    with b.Sim(c1["N"], c1["L"]) as s:
+        s.set_state(c1["pos"], c1["vel"])
+        s.step(100, 0)
+        p, v = s.get_state()
+        s.set_state(p, -v)
+        s.step(100, 0)
+        p2, v2 = s.get_state()
+    d = p2.astype(np.float64) - c1["pos"]
+    d -= c1["L"] * np.rint(d / c1["L"])
+    assert np.max(np.abs(d)) < 1e-3                      # R19: FP32 returns to ~1e-4
+
+
+def test_melted_snapshot_n4000(b, oracle_uniforms):
+    """Forces on a melted N = 4000 snapshot (pair forces up to ~70), both algos."""
+    pos, L = wl.fcc_positions(10, 0.8)
+    x0 = wl.splitmix64(77) & wl.MASK48
+    vel = wl.maxwell_boltzmann(oracle_uniforms(x0, 6 * 4000), 4000, 1.0)
+    with b.Sim(4000, L) as s:
+        s.set_state(pos, vel)
+        s.step(400, b.MD_CELL)
+        p, v = s.get_state()
+        Fo, peo, wo = oracle.forces(p.astype(np.float64), L, algo=1)
+        assert np.max(np.abs(Fo)) > 30
+        for algo in (0, 1):
+            s.set_state(p, v)
+            s.compute_forces(algo)
+            nviol, worst = force_check(s.forces(), Fo)
+            assert nviol == 0, (algo, nviol, worst)
+            ke, pe, w = s.energies()
+            assert pe == pytest.approx(peo, rel=1e-9) and w == pytest.approx(wo, rel=1e-9)
+            assert ke == pytest.approx(oracle.kinetic_energy(v.astype(np.float64)), rel=1e-9)

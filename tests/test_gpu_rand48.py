@@ -1,0 +1,104 @@
+"""rand48 on the GPU is bit-exact against the sequential oracle (gpu-marked), including
+across skip-ahead boundaries, ragged tails, unaligned outputs and host/device buffers."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_0709_3225_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def b():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_0709_3225_b200 import binding
+    return binding
+
+
+@pytest.mark.parametrize("kind", [0, 1, 2, 3])
+@pytest.mark.parametrize("nstreams,ndraws", [(1, 1), (3, 5), (7, 127), (5, 128), (4, 129), (2, 1000),
+                                             (33, 1024), (17, 4096), (2, 4099), (1, 300001), (600, 260)])
+def test_bit_exact_vs_sequential(b, kind, nstreams, ndraws):
+    seeds = wl.stream_seeds(wl.MASTER_SEED + nstreams, nstreams)
+    ref, ref_state = oracle.rand48_fill(seeds, ndraws, kind)
+    out, state = b.rand48(seeds, ndraws, kind)
+    assert out.dtype == ref.dtype
+    assert np.array_equal(out.view(np.uint8), ref.view(np.uint8))
+    assert np.array_equal(state, ref_state)
+
+
+def test_edge_seeds(b):
+    seeds = np.array([0, 1, (1 << 48) - 1, 0x1234ABCD330E, 0x330E], dtype=np.uint64)
+    for kind in range(4):
+        ref, rs = oracle.rand48_fill(seeds, 777, kind)
+        out, st = b.rand48(seeds, 777, kind)
+        assert np.array_equal(out.view(np.uint8), ref.view(np.uint8)) and np.array_equal(st, rs)
+    with pytest.raises(b.MDError) as e:
+        b.rand48(np.array([1 << 48], dtype=np.uint64), 4)
+    assert e.value.code == b.MD_EINVAL
+
+
+def test_consecutive_calls_concatenate(b):
+    seeds = wl.stream_seeds(5, 9)
+    a, s1 = b.rand48(seeds, 1000, 0)
+    c, s2 = b.rand48(s1, 531, 0)
+    ref, rs = oracle.rand48_fill(seeds, 1531, 0)
+    assert np.array_equal(np.concatenate([a, c], axis=1), ref) and np.array_equal(s2, rs)
+
+
+def test_device_buffers_and_unaligned_output(b):
+    import torch
+    seeds = wl.stream_seeds(11, 6)
+    nd = 2051
+    ref, rs = oracle.rand48_fill(seeds, nd, 0)
+    dseeds = torch.from_numpy(seeds.astype(np.int64)).cuda()
+    buf = torch.zeros(6 * nd + 1, dtype=torch.int32, device="cuda")
+    out = buf[1:]                                           # 4-byte aligned only
+    b.rand48_fill(dseeds.data_ptr(), 6, nd, 0, out.data_ptr())
+    assert np.array_equal(out.cpu().numpy().view(np.uint32).reshape(6, nd), ref)
+    assert np.array_equal(dseeds.cpu().numpy().view(np.uint64), rs)
+    bad = torch.tensor([1 << 50], dtype=torch.int64, device="cuda")
+    assert b._lib.rand48_fill(bad.data_ptr(), 1, 4, 0, out.data_ptr()) == b.MD_EINVAL
+
+
+def test_single_stream_skip_ahead_2p24(b):
+    """One stream split across ~8000 warps by skip-ahead (config 5 part 2 at 1/16 size)."""
+    x0 = wl.splitmix64(wl.MASTER_SEED) & wl.MASK48
+    n = 1 << 24
+    for kind in (0, 2):
+        ref, rs = oracle.rand48_fill([x0], n, kind)
+        out, st = b.rand48([x0], n, kind)
+        assert np.array_equal(out.view(np.uint8), ref.view(np.uint8)) and st[0] == rs[0]
+    assert int(st[0]) == oracle.rand48_skip(x0, n)
+
+
+def test_config5_sampled_full_size(b):
+    """BASELINE config 5 at full size on device buffers; sampled streams and windows are
+    compared with the sequential oracle, final states with its skip-ahead."""
+    import torch
+    ns, nd = wl.C5_NSTREAMS, wl.C5_NDRAWS
+    seeds = wl.stream_seeds(wl.MASTER_SEED, ns)
+    for kind, tdt in ((0, torch.int32), (2, torch.float64)):
+        dseeds = torch.from_numpy(seeds.astype(np.int64)).cuda()
+        out = torch.empty(ns * nd, dtype=tdt, device="cuda")
+        b.rand48_fill(dseeds.data_ptr(), ns, nd, kind, out.data_ptr())
+        pick = [0, 1, 777, 32768, ns - 1]
+        ref, rs = oracle.rand48_fill(seeds[pick], nd, kind)
+        got = out.view(ns, nd)[pick].cpu().numpy()
+        assert np.array_equal(got.view(np.uint8), ref.view(np.uint8))
+        st = dseeds.cpu().numpy().view(np.uint64)
+        assert np.array_equal(st[pick], rs)
+        assert all(int(st[i]) == oracle.rand48_skip(int(seeds[i]), nd) for i in range(0, ns, 997))
+    # single stream of 2^28 draws: windows around segment boundaries + the tail
+    n = wl.C5_SINGLE_NDRAWS
+    x0 = int(seeds[0])
+    d1 = torch.tensor([x0], dtype=torch.int64, device="cuda")
+    out = torch.empty(n, dtype=torch.int32, device="cuda")
+    b.rand48_fill(d1.data_ptr(), 1, n, 0, out.data_ptr())
+    for start in (0, 2047, 2048, 4096 * 1000 - 3, n // 2 - 100, n - 5000):
+        cnt = min(5000, n - start)
+        ref, _ = oracle.rand48_fill([oracle.rand48_skip(x0, start)], cnt, 0)
+        assert np.array_equal(out[start:start + cnt].cpu().numpy().view(np.uint32), ref[0]), start
+    assert int(d1.cpu().numpy().view(np.uint64)[0]) == oracle.rand48_skip(x0, n)
