@@ -1,0 +1,371 @@
+#!/usr/bin/env python
+"""Benchmark of the LJ MD hot path (arXiv 0709.3225) on B200, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload c2_allpairs_32k|c3_cell_256k|c4a_cell_2048k|...] [--no-others]
+
+A "step" is one velocity-Verlet step of the named workload (half-kick, drift + wrap, [cell
+build,] force + PE + virial, half-kick + KE, reductions).  The headline workload is
+BASELINE.json configs[1] (N = 32000, all-pairs); the cell-list configs and the rand48 config
+are measured in the same run and reported under "others" (skip with --no-others).
+Multi-GPU: the path does not shard in this build ("replicas only"):
+under torchrun every rank runs an independent replica and `value` is the aggregate.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_0709_3225_b200 import workloads as wl  # noqa: E402
+
+FP32_LANES_PER_SM = 128
+FLOP_PER_PAIR_TEST = 8.0        # 3 sub + 1 mul + 2 fma; the compare is not a flop
+FLOP_PER_INRANGE = 19.0
+NBR_PER_ATOM = lambda rho, rc: 4.0 / 3.0 * np.pi * rc ** 3 * rho  # noqa: E731
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=d["hbm_gbs"], sm_max_mhz=d.get("sm_max_mhz", 1965.0), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.25)
+            self.proc.terminate()
+            self.thr.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])), mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v == "Active":
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+# ----------------------------------------------------------------------------- our arm
+def flush_l2(torch, buf):
+    buf.add_(1)           # read + write 256 MB: larger than the 126 MB L2
+
+
+def time_md(b, torch, sysd, algo, steps, warmup, flush, buf):
+    """Returns dict with ms_per_step (flushed per-step timing), steady ms_per_step
+    (md_step(K) back to back), per-phase times and kernel-launch counts."""
+    N = sysd["N"]
+    s = b.Sim(N, sysd["L"], rc=sysd["rc"], eps=sysd["eps"], sigma=sysd["sigma"], dt=sysd["dt"],
+              shifted=sysd["shifted"])
+    s.set_state(sysd["pos"], sysd["vel"])
+    s.step(warmup, algo)
+    torch.cuda.synchronize()
+    # (1) steady state: K steps in one call, the way a user runs MD
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = s.stat("kernel_launches")
+    e0.record()
+    s.step(steps, algo)
+    e1.record()
+    torch.cuda.synchronize()
+    steady_ms = e0.elapsed_time(e1) / steps
+    launches = int(s.stat("kernel_launches") - l0)
+    # (2) per-phase kernel timing with CUDA events inside the library (same stream)
+    s.option("time_kernels", 1)
+    s.step(steps, algo)
+    t_force = s.stat("t_force_ms") / max(1.0, s.stat("n_force"))
+    phases = {k: s.stat("t_%s_ms" % k) / steps for k in ("integrate", "build", "force", "other")}
+    s.option("time_kernels", 0)
+    # (3) cold-L2 per-step timing: flush between steps, each step its own md_step(1)
+    flushed_ms = None
+    if flush:
+        tot = 0.0
+        for _ in range(steps):
+            flush_l2(torch, buf)
+            e0.record()
+            s.step(1, algo)
+            e1.record()
+            torch.cuda.synchronize()
+            tot += e0.elapsed_time(e1)
+        flushed_ms = tot / steps
+    ke, pe, w = s.energies()
+    s.close()
+    return dict(steady_ms=steady_ms, flushed_ms=flushed_ms, launches_per_step=launches / steps,
+                t_force_kernel_ms=t_force, phases_ms=phases, energy=ke + pe)
+
+
+def time_md_e2e(b, torch, sysd, algo, steps):
+    """End to end through the C ABI with HOST (pinned) buffers: every step uploads the state,
+    advances one step and reads the state and energies back."""
+    N = sysd["N"]
+    pos = torch.from_numpy(sysd["pos"].copy()).pin_memory()
+    vel = torch.from_numpy(sysd["vel"].copy()).pin_memory()
+    s = b.Sim(N, sysd["L"], rc=sysd["rc"], eps=sysd["eps"], sigma=sysd["sigma"], dt=sysd["dt"],
+              shifted=sysd["shifted"])
+    h = s.h
+    for it in range(steps + 2):
+        if it == 2:
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+        b.md_set_state(h, pos, vel)
+        b.md_step(h, 1, algo)
+        b.md_get_state(h, pos, vel)
+        b.md_get_energies(h)
+    torch.cuda.synchronize()
+    dt = (time.perf_counter() - t0) / steps
+    s.close()
+    return dict(ms_per_step=dt * 1e3, h2d=2 * N * 12, d2h=2 * N * 12 + 24)
+
+
+def allpairs_roofline(N, rho, rc, t_kernel_ms, peaks, n_sms):
+    pairs = float(N) * (N - 1)
+    flops = pairs * FLOP_PER_PAIR_TEST + N * NBR_PER_ATOM(rho, rc) * FLOP_PER_INRANGE
+    peak = n_sms * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    ach = flops / (t_kernel_ms * 1e-3) / 1e12
+    return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+            "kernel": "all-pairs force", "pair_tests_per_s": pairs / (t_kernel_ms * 1e-3),
+            "peak_source": "derived: SMs x 128 FP32 lanes x 2 x clocks.max.sm (DESIGN.md section 8)"}
+
+
+def cell_roofline(N, rho, rc, ncell, t_kernel_ms, peaks, n_sms):
+    cand = 27.0 * N / ncell ** 3 * N                    # ordered candidate pairs per launch
+    flops = cand * FLOP_PER_PAIR_TEST + N * NBR_PER_ATOM(rho, rc) * FLOP_PER_INRANGE
+    peak = n_sms * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    ach = flops / (t_kernel_ms * 1e-3) / 1e12
+    return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+            "kernel": "cell-list force", "candidate_tests_per_s": cand / (t_kernel_ms * 1e-3)}
+
+
+def bench_rand48(b, torch, steps, peaks):
+    """Config 5: 65536 streams x 4096 draws and one stream of 2^28 draws, uint32 and double."""
+    res = {}
+    seeds0 = torch.from_numpy(wl.stream_seeds(wl.MASTER_SEED, wl.C5_NSTREAMS).astype(np.int64)).cuda()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for name, ns, nd in (("streams_65536x4096", wl.C5_NSTREAMS, wl.C5_NDRAWS), ("single_2p28", 1, wl.C5_SINGLE_NDRAWS)):
+        for kind, tdt, esz in ((0, torch.int32, 4), (2, torch.float64, 8)):
+            out = torch.empty(ns * nd, dtype=tdt, device="cuda")     # 1.07 / 2.15 GB > L2
+            seeds = seeds0[:ns].clone()
+            for _ in range(2):
+                b.rand48_fill(seeds.data_ptr(), ns, nd, kind, out.data_ptr())
+            e0.record()
+            for _ in range(steps):
+                b.rand48_fill(seeds.data_ptr(), ns, nd, kind, out.data_ptr())
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / steps
+            gbs = ns * nd * esz / (ms * 1e-3) / 1e9
+            res["%s_%s" % (name, "u32" if kind == 0 else "f64")] = {
+                "draws_per_s": ns * nd / (ms * 1e-3), "ms": ms, "store_GBps": gbs,
+                "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                             "frac": gbs / peaks["hbm_gbs"], "traffic": None}}
+            del out
+    return res
+
+
+def gpu_uniform_source(b):
+    def src(seed48, n):
+        out, _ = b.rand48([seed48], n, b.R48_F64)
+        return out[0]
+    return src
+
+
+def cpu_baseline_md(sysd, algo, budget_steps):
+    """The oracle as it stands, timed on this box's host cores on a bounded sample."""
+    import oracle
+    ncores = os.cpu_count() or 1
+    threads = ncores if algo == 1 else 1          # only the cell-list loop has an OpenMP pragma
+    oracle.set_threads(threads)
+    pos, vel = sysd["pos"].astype(np.float64), sysd["vel"].astype(np.float64)
+    t0 = time.perf_counter()
+    oracle.verlet_run(pos, vel, sysd["L"], budget_steps, rc=sysd["rc"], eps=sysd["eps"], sigma=sysd["sigma"],
+                      dt=sysd["dt"], mode=sysd["shifted"], algo=algo)
+    dt = time.perf_counter() - t0
+    evals = budget_steps + 1                        # verlet_run evaluates forces once at entry
+    return dict(value=sysd["N"] * evals / dt, seconds=dt, cores=threads, evals=evals)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank, local_rank, world = dist_env()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_0709_3225_b200 import binding as b
+    peaks = measured_peaks()
+    props = torch.cuda.get_device_properties(local_rank)
+    n_sms = props.multi_processor_count
+    name = args.workload
+    cfg = wl.CONFIGS[name]
+    sysd = wl.md_system(name, gpu_uniform_source(b))
+    algo = cfg["algo"]
+    buf = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")
+    steps, warmup = args.steps, max(3, args.warmup)
+
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    with ClockSampler(local_rank) as clk:
+        r = time_md(b, torch, sysd, algo, steps, warmup, True, buf)
+    ms = r["flushed_ms"]
+    e2e = time_md_e2e(b, torch, sysd, algo, min(steps, 50))
+    if world > 1:
+        t = torch.tensor([ms, r["steady_ms"], e2e["ms_per_step"]], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, r["steady_ms"], e2e["ms_per_step"] = [float(x) for x in t.cpu()]
+    N = sysd["N"]
+    value = world * N / (ms * 1e-3)
+    if algo == 0:
+        roof = allpairs_roofline(N, cfg["rho"], wl.RC, r["t_force_kernel_ms"], peaks, n_sms)
+    else:
+        with b.Sim(N, sysd["L"]) as tmp:
+            ncell = int(tmp.stat("ncell"))
+        roof = cell_roofline(N, cfg["rho"], wl.RC, ncell, r["t_force_kernel_ms"], peaks, n_sms)
+    roof["kernel_ms"] = r["t_force_kernel_ms"]
+    roof["kernel_share_of_step"] = r["phases_ms"]["force"] / max(1e-12, sum(r["phases_ms"].values()))
+
+    line = {
+        "metric": "LJ MD atom-steps/s", "value": value, "unit": "atom-steps/s", "n_gpus": world, "steps": steps,
+        "warmup": warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32 state and distance filter, f64 in-range pair terms",
+        "data": "synthetic",
+        "config": {"workload": name, "N": N, "rho": cfg["rho"], "T": cfg["T"], "rc": wl.RC, "dt": wl.DT,
+                   "algo": "allpairs" if algo == 0 else "cell", "shifted": wl.SHIFTED,
+                   "l2": "flushed between steps (256 MB read-modify-write); steady_state is the unflushed md_step(K) loop",
+                   "parallelism": "replicas x%d" % world if world > 1 else "single GPU"},
+        "steady_state": {"ms_per_step": r["steady_ms"], "value": world * N / (r["steady_ms"] * 1e-3)},
+        "phases_ms": r["phases_ms"],
+        "roofline": roof,
+        "e2e": {"value": world * N / (e2e["ms_per_step"] * 1e-3), "unit": "atom-steps/s",
+                "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"], "ms_per_step": e2e["ms_per_step"]},
+        "gpu_launches": int(round(r["launches_per_step"] * steps)),
+        "clocks": clk.summary(),
+        "peaks": peaks,
+    }
+    if rank == 0 and world == 1:
+        nb = 2 if algo == 0 and N >= 20000 else (20 if N <= 4000 else 3)
+        cb = cpu_baseline_md(sysd, algo, nb)
+        line["cpu_baseline"] = {"value": cb["value"], "unit": "atom-steps/s", "cores": cb["cores"], "kind": "oracle",
+                                "sample": "%d force evaluations (%d velocity-Verlet steps) of the same N=%d system, %.1f s"
+                                          % (cb["evals"], nb, N, cb["seconds"])}
+    if rank == 0 and world == 1 and not args.no_others:
+        others = {}
+        for oname in ("c1_allpairs_500", "c3_cell_256k", "c4a_cell_2048k", "c4b_cell_2048k_rho03"):
+            if oname == name:
+                continue
+            ocfg = wl.CONFIGS[oname]
+            osys = wl.md_system(oname, gpu_uniform_source(b))
+            osteps = 200 if ocfg["n"] <= 5 else (20 if ocfg["n"] >= 80 else 50)
+            rr = time_md(b, torch, osys, ocfg["algo"], osteps, 5, False, buf)
+            others[oname] = {"N": osys["N"], "atom_steps_per_s": osys["N"] / (rr["steady_ms"] * 1e-3),
+                             "ms_per_step": rr["steady_ms"], "phases_ms": rr["phases_ms"],
+                             "force_kernel_ms": rr["t_force_kernel_ms"],
+                             "launches_per_step": rr["launches_per_step"]}
+        others["c5_rand48"] = bench_rand48(b, torch, 5, peaks)
+        line["others"] = others
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------- reference arm
+def run_reference(args):
+    """The oracle as it stands on the host cores, same config/metric (bounded sample per step)."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    import oracle
+    name = args.workload
+    cfg = wl.CONFIGS[name]
+
+    def src(seed48, n):
+        return oracle.rand48_fill([seed48], n, 2)[0][0]
+    sysd = wl.md_system(name, src)
+    algo, N = cfg["algo"], sysd["N"]
+    threads = (os.cpu_count() or 1) if algo == 1 else 1
+    oracle.set_threads(threads)
+    pos, vel = sysd["pos"].astype(np.float64), sysd["vel"].astype(np.float64)
+    steps, warmup = max(1, min(args.steps, 3)), min(args.warmup, 1)
+    pos, vel, _, _ = oracle.verlet_run(pos, vel, sysd["L"], warmup, algo=algo) if warmup else (pos, vel, None, None)
+    t0 = time.perf_counter()
+    oracle.verlet_run(pos, vel, sysd["L"], steps, algo=algo)
+    dt = time.perf_counter() - t0
+    evals = steps + 1
+    value = N * evals / dt
+    line = {"impl": "reference", "metric": "LJ MD atom-steps/s", "value": value, "unit": "atom-steps/s",
+            "n_gpus": world, "steps": steps, "warmup": warmup, "ms_per_step": dt / evals * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "N": N, "rho": cfg["rho"], "T": cfg["T"], "rc": wl.RC, "dt": wl.DT,
+                       "algo": "allpairs" if algo == 0 else "cell", "shifted": wl.SHIFTED},
+            "cpu_baseline": {"value": value, "unit": "atom-steps/s", "kind": "oracle", "cores": threads,
+                             "sample": "%d force evaluations of the same N=%d system (steps clamped to 3 so the run "
+                                       "ends within minutes)" % (evals, N)},
+            "e2e": {"value": value, "unit": "atom-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c2_allpairs_32k", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--no-others", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

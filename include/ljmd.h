@@ -111,6 +111,9 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
 
 /* Tuning and introspection.  md_set_option keys:
  *   "graph"          1 (default) replay each step from a CUDA graph, 0 launch directly
+ *   "time_kernels"   1 = record CUDA events around every phase of md_step (disables the graph);
+ *                    read back with md_get_stat "t_force_ms", "t_build_ms", "t_integrate_ms",
+ *                    "t_other_ms", "n_force"; setting it resets the accumulators
  *   "precise_r2"     squared distance below which the pair term is evaluated in FP64
  *                    (default: all in-range pairs); 0 = FP32 everywhere
  *   "sort_every"     all-pairs path: re-sort atoms spatially every k steps (default 20)

@@ -183,6 +183,7 @@ int ljmd_forces_cell(md_sim *s)
     double *pw = s->part + 2 * (size_t)s->part_cap;
     k_force_cell<<<nb, CF_T, 0, s->stream>>>(s->lpos, s->cell_start, N, s->grid, s->pp, s->frc, ppe, pw);
     CKL(s);
+    ljmd_tick(s, TAG_FORCE);
     s->n_pe = nb;
     return MD_OK;
 }

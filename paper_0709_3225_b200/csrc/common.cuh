@@ -79,7 +79,19 @@ struct md_sim {
     // CUDA graph cache for one step
     cudaGraphExec_t graph_exec[2];
     bool graph_ok[2];
+    // optional per-phase timing with CUDA events on s->stream ("time_kernels" option)
+    bool time_kernels;
+    cudaEvent_t *ev_pool;
+    int *ev_tag;
+    int ev_cap, ev_n;
+    double t_phase[4];            // ms: integrate, build, force kernel, other
+    int64_t n_phase[4];
 };
+
+enum { TAG_START = -1, TAG_INTEGRATE = 0, TAG_BUILD = 1, TAG_FORCE = 2, TAG_OTHER = 3 };
+// Record an event; the time since the previous tick is attributed to `tag`.
+void ljmd_tick(md_sim *s, int tag);
+int ljmd_collect_ticks(md_sim *s);
 
 // ---- kernels' host launchers (each returns md_status) ---------------------------
 int ljmd_pack_state(md_sim *s, const float *dpos, const float *dvel);

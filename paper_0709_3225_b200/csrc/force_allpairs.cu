@@ -96,8 +96,10 @@ int ljmd_forces_allpairs(md_sim *s)
     k_force_allpairs_general<<<grid, AP_T, 0, s->stream>>>(
         s->pos, N, s->pp, s->Lf, 1.0f / s->Lf, s->L, 1.0 / s->L, jchunk, s->fpart, ppe, pw);
     CKL(s);
+    ljmd_tick(s, TAG_FORCE);
     s->n_pe = niblk * nsplit;
     k_combine_forces<<<(N + 255) / 256, 256, 0, s->stream>>>(s->frc, s->fpart, N, nsplit);
     CKL(s);
+    ljmd_tick(s, TAG_OTHER);
     return MD_OK;
 }

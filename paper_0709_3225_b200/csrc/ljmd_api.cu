@@ -122,12 +122,49 @@ static void setup_pair(md_sim *s)
     P.f_rcf = (float)P.f_rc;
 }
 
+// ---- per-phase timing -------------------------------------------------------------------
+void ljmd_tick(md_sim *s, int tag)
+{
+    if (!s->time_kernels) return;
+    if (s->ev_n == s->ev_cap) {
+        int cap = s->ev_cap ? 2 * s->ev_cap : 1024;
+        cudaEvent_t *p = (cudaEvent_t *)realloc(s->ev_pool, cap * sizeof(cudaEvent_t));
+        int *t = (int *)realloc(s->ev_tag, cap * sizeof(int));
+        if (!p || !t) return;
+        s->ev_pool = p;
+        s->ev_tag = t;
+        for (int k = s->ev_cap; k < cap; k++) cudaEventCreate(&s->ev_pool[k]);
+        s->ev_cap = cap;
+    }
+    cudaEventRecord(s->ev_pool[s->ev_n], s->stream);
+    s->ev_tag[s->ev_n++] = tag;
+}
+
+int ljmd_collect_ticks(md_sim *s)
+{
+    if (!s->time_kernels || s->ev_n == 0) return MD_OK;
+    CK(cudaStreamSynchronize(s->stream));
+    for (int k = 1; k < s->ev_n; k++) {
+        int tag = s->ev_tag[k];
+        if (tag < 0) continue;
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, s->ev_pool[k - 1], s->ev_pool[k]));
+        s->t_phase[tag] += ms;
+        s->n_phase[tag]++;
+    }
+    s->ev_n = 0;
+    return MD_OK;
+}
+
 // ---- create / destroy -----------------------------------------------------------------
 static void free_all(md_sim *s)
 {
     cudaStream_t st = s->stream;
     for (int k = 0; k < 2; k++)
         if (s->graph_exec[k]) cudaGraphExecDestroy(s->graph_exec[k]);
+    for (int k = 0; k < s->ev_cap; k++) cudaEventDestroy(s->ev_pool[k]);
+    free(s->ev_pool);
+    free(s->ev_tag);
     void *ptrs[] = {s->pos, s->vel, s->frc, s->pos2, s->vel2, s->lpos, s->cell_of, s->rank, s->cell_count,
                     s->cell_start, s->max_occ, s->fpart, s->part, s->energies, s->xfer};
     for (void *p : ptrs) ljmd_dev_free(p, st);
@@ -309,6 +346,7 @@ static int eval_forces(md_sim *s, int algo)
     int r;
     if (algo == MD_CELL) {
         if ((r = ljmd_cell_build(s))) return r;
+        ljmd_tick(s, TAG_BUILD);
         if ((r = ljmd_forces_cell(s))) return r;
     } else {
         s->layout_cell = false;
@@ -344,12 +382,17 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
         s->forces_valid = true;
         s->forces_algo = algo;
     }
+    ljmd_tick(s, TAG_START);
     for (int64_t k = 0; k < nsteps; k++) {
         if ((r = ljmd_kick_drift(s))) return r;
+        ljmd_tick(s, TAG_INTEGRATE);
         if ((r = eval_forces(s, algo))) return r;
         if ((r = ljmd_kick_ke(s))) return r;
+        ljmd_tick(s, TAG_INTEGRATE);
     }
     if ((r = ljmd_reduce_energies(s))) return r;
+    ljmd_tick(s, TAG_OTHER);
+    if ((r = ljmd_collect_ticks(s))) return r;
     CK(cudaStreamSynchronize(s->stream));
     s->forces_algo = algo;
     s->steps_done += nsteps;
@@ -361,6 +404,11 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
 {
     if (!s || !key) return MD_EINVAL;
     if (!strcmp(key, "graph")) s->use_graph = value != 0.0;
+    else if (!strcmp(key, "time_kernels")) {
+        s->time_kernels = value != 0.0;
+        s->ev_n = 0;
+        for (int k = 0; k < 4; k++) { s->t_phase[k] = 0.0; s->n_phase[k] = 0; }
+    }
     else if (!strcmp(key, "precise_r2")) {
         if (!(value >= 0)) return MD_EINVAL;
         s->pp.precise_r2 = value;
@@ -381,6 +429,11 @@ extern "C" int md_get_stat(md_sim *s, const char *key, double *value)
     else if (!strcmp(key, "kernel_launches")) *value = (double)s->launches;
     else if (!strcmp(key, "steps_done")) *value = (double)s->steps_done;
     else if (!strcmp(key, "ap_nsplit")) *value = s->ap_nsplit;
+    else if (!strcmp(key, "t_integrate_ms")) *value = s->t_phase[TAG_INTEGRATE];
+    else if (!strcmp(key, "t_build_ms")) *value = s->t_phase[TAG_BUILD];
+    else if (!strcmp(key, "t_force_ms")) *value = s->t_phase[TAG_FORCE];
+    else if (!strcmp(key, "t_other_ms")) *value = s->t_phase[TAG_OTHER];
+    else if (!strcmp(key, "n_force")) *value = (double)s->n_phase[TAG_FORCE];
     else if (!strcmp(key, "max_occupancy")) {
         int h = 0;
         CK(cudaMemcpyAsync(&h, s->max_occ, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
