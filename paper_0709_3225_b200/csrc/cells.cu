@@ -104,20 +104,27 @@ k_scatter(const float4 *__restrict__ pos, const float4 *__restrict__ vel, int N,
     lpos[dst] = l;
 }
 
+int ljmd_scan_counts(md_sim *s, int *count, int *start, int n)
+{
+    k_scan_cells<<<1, 1024, 0, s->stream>>>(count, start, n, s->max_occ);
+    CKL(s);
+    return MD_OK;
+}
+
 int ljmd_cell_build(md_sim *s)
 {
     int N = (int)s->N;
     int nb = (N + CB_T - 1) / CB_T;
     k_bin<<<nb, CB_T, 0, s->stream>>>(s->pos, N, s->grid, s->cell_of, s->rank, s->cell_count);
     CKL(s);
-    k_scan_cells<<<1, 1024, 0, s->stream>>>(s->cell_count, s->cell_start, s->grid.ncells, s->max_occ);
-    CKL(s);
+    int r = ljmd_scan_counts(s, s->cell_count, s->cell_start, s->grid.ncells);
+    if (r) return r;
     k_scatter<<<nb, CB_T, 0, s->stream>>>(s->pos, s->vel, N, s->grid, s->cell_of, s->rank, s->cell_start,
                                          s->pos2, s->vel2, s->lpos);
     CKL(s);
     float4 *t = s->pos; s->pos = s->pos2; s->pos2 = t;
     t = s->vel; s->vel = s->vel2; s->vel2 = t;
-    s->layout_cell = true;
+    s->layout = LAYOUT_CELL;
     return MD_OK;
 }
 

@@ -63,14 +63,19 @@ struct md_sim {
     int *max_occ;                 // [1]
     // all-pairs partial forces: [nsplit][3][N] doubles
     double *fpart;
-    int ap_nsplit;
+    int ap_nsplit;                // j splits of the general kernel
+    // all-pairs tiled kernel: spatial tiles ta x tb x tc, j splits, validity bound
+    bool ap_tiled, ap_force_general;
+    int ap_ta, ap_tb, ap_tc, ap_ntiles, ap_tsplit, ap_since_sort;
+    float ap_hmax;
+    int *tile_count, *tile_start;
     // energy partials and results
     double *part;                 // [3][part_cap] block partials: KE, PE, W
     int part_cap;
     int n_ke, n_pe;               // valid partial counts
     double *energies;             // [3] on device: KE, PE, W
     float *xfer;                  // [N][3] staging for host/device packing
-    bool layout_cell;             // slot order is cell-sorted and lpos/cell_start are current
+    int layout;                   // LAYOUT_*: how the slots are currently ordered
     bool has_state, forces_valid;
     int forces_algo;
     bool use_graph;
@@ -88,6 +93,7 @@ struct md_sim {
     int64_t n_phase[4];
 };
 
+enum { LAYOUT_NONE = 0, LAYOUT_CELL = 1, LAYOUT_TILE = 2 };
 enum { TAG_START = -1, TAG_INTEGRATE = 0, TAG_BUILD = 1, TAG_FORCE = 2, TAG_OTHER = 3 };
 // Record an event; the time since the previous tick is attributed to `tag`.
 void ljmd_tick(md_sim *s, int tag);
@@ -101,6 +107,8 @@ int ljmd_kick_ke(md_sim *s);
 int ljmd_ke_only(md_sim *s);
 int ljmd_reduce_energies(md_sim *s);
 int ljmd_forces_allpairs(md_sim *s);
+void ljmd_ap_plan(md_sim *s);
+int ljmd_scan_counts(md_sim *s, int *count, int *start, int n);   // exclusive scan, zeroes count
 int ljmd_cell_build(md_sim *s);
 int ljmd_forces_cell(md_sim *s);
 

@@ -166,7 +166,8 @@ static void free_all(md_sim *s)
     free(s->ev_pool);
     free(s->ev_tag);
     void *ptrs[] = {s->pos, s->vel, s->frc, s->pos2, s->vel2, s->lpos, s->cell_of, s->rank, s->cell_count,
-                    s->cell_start, s->max_occ, s->fpart, s->part, s->energies, s->xfer};
+                    s->cell_start, s->max_occ, s->fpart, s->part, s->energies, s->xfer, s->tile_count,
+                    s->tile_start};
     for (void *p : ptrs) ljmd_dev_free(p, st);
 }
 
@@ -197,7 +198,7 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->dtf = (float)dt;
     s->hdtf = (float)(0.5 * dt);
     s->use_graph = true;
-    s->sort_every = 20;
+    s->sort_every = 10;
     setup_grid(s);
     setup_pair(s);
 
@@ -208,7 +209,10 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     if (nsplit > 64) nsplit = 64;
     if (nsplit < 1) nsplit = 1;
     s->ap_nsplit = nsplit;
+    ljmd_ap_plan(s);
     int cap_ap = niblk * nsplit;
+    if (s->ap_tiled && s->ap_ntiles * s->ap_tsplit > cap_ap) cap_ap = s->ap_ntiles * s->ap_tsplit;
+    if (s->ap_tiled && s->ap_tsplit > nsplit) nsplit = s->ap_tsplit;      // fpart holds either kernel's splits
     int cap_it = (int)((N + 255) / 256);
     s->part_cap = (cap_ap > cap_it ? cap_ap : cap_it) + 64;
 
@@ -230,7 +234,10 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->part = (double *)ljmd_dev_alloc((size_t)3 * s->part_cap * sizeof(double), st);
     s->energies = (double *)ljmd_dev_alloc(3 * sizeof(double), st);
     s->xfer = (float *)ljmd_dev_alloc((size_t)N * 3 * sizeof(float), st);
-    if (!s->pos || !s->vel || !s->frc || !s->pos2 || !s->vel2 || !s->lpos || !s->cell_of || !s->rank ||
+    int ntiles = s->ap_tiled ? s->ap_ntiles : 1;
+    s->tile_count = (int *)ljmd_dev_alloc((size_t)ntiles * sizeof(int), st);
+    s->tile_start = (int *)ljmd_dev_alloc(((size_t)ntiles + 1) * sizeof(int), st);
+    if (!s->tile_count || !s->tile_start || !s->pos || !s->vel || !s->frc || !s->pos2 || !s->vel2 || !s->lpos || !s->cell_of || !s->rank ||
         !s->cell_count || !s->cell_start || !s->max_occ || !s->fpart || !s->part || !s->energies || !s->xfer) {
         free_all(s);
         delete s;
@@ -238,6 +245,7 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     }
     cudaError_t e = cudaMemsetAsync(s->cell_count, 0, (size_t)ncells * sizeof(int), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->max_occ, 0, sizeof(int), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->tile_count, 0, (size_t)ntiles * sizeof(int), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->frc, 0, f4, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) {
@@ -290,7 +298,7 @@ extern "C" int md_set_state(md_sim *s, const float *pos, const float *vel)
     CK(cudaStreamSynchronize(s->stream));
     s->has_state = true;
     s->forces_valid = false;
-    s->layout_cell = false;
+    s->layout = LAYOUT_NONE;
     return MD_OK;
 }
 
@@ -349,7 +357,6 @@ static int eval_forces(md_sim *s, int algo)
         ljmd_tick(s, TAG_BUILD);
         if ((r = ljmd_forces_cell(s))) return r;
     } else {
-        s->layout_cell = false;
         if ((r = ljmd_forces_allpairs(s))) return r;
     }
     return MD_OK;
@@ -412,6 +419,8 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
     else if (!strcmp(key, "precise_r2")) {
         if (!(value >= 0)) return MD_EINVAL;
         s->pp.precise_r2 = value;
+    } else if (!strcmp(key, "ap_general")) {
+        s->ap_force_general = value != 0.0;
     } else if (!strcmp(key, "sort_every")) {
         if (value < 1) return MD_EINVAL;
         s->sort_every = (int)value;
@@ -429,6 +438,9 @@ extern "C" int md_get_stat(md_sim *s, const char *key, double *value)
     else if (!strcmp(key, "kernel_launches")) *value = (double)s->launches;
     else if (!strcmp(key, "steps_done")) *value = (double)s->steps_done;
     else if (!strcmp(key, "ap_nsplit")) *value = s->ap_nsplit;
+    else if (!strcmp(key, "ap_tiled")) *value = s->ap_tiled ? 1 : 0;
+    else if (!strcmp(key, "ap_ntiles")) *value = s->ap_ntiles;
+    else if (!strcmp(key, "ap_tsplit")) *value = s->ap_tsplit;
     else if (!strcmp(key, "t_integrate_ms")) *value = s->t_phase[TAG_INTEGRATE];
     else if (!strcmp(key, "t_build_ms")) *value = s->t_phase[TAG_BUILD];
     else if (!strcmp(key, "t_force_ms")) *value = s->t_phase[TAG_FORCE];
