@@ -116,8 +116,10 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
  *                    "t_other_ms", "n_force"; setting it resets the accumulators
  *   "precise_r2"     squared distance below which the pair term is evaluated in FP64
  *                    (default: all in-range pairs); 0 = FP32 everywhere
- *   "sort_every"     all-pairs path: re-sort atoms into spatial tiles every k steps (default 10)
+ *   "sort_every"     all-pairs path: re-sort atoms along the Hilbert curve every k steps (default 10)
  *   "ap_general"     1 = force the unsorted per-pair-minimum-image all-pairs kernel
+ *   "ap_R"           atoms per thread (1, 2, 4, 8) of the sorted all-pairs kernel, overriding the
+ *                    choice made from N and L; blocks too wide for the box test per-pair images
  * md_get_stat keys: "ncell" (cells per dimension), "max_occupancy", "kernel_launches"
  * (kernels launched by this handle so far), "steps_done", "side" (cell side). */
 int md_set_option(md_sim *s, const char *key, double value);

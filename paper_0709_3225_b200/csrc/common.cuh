@@ -64,9 +64,10 @@ struct md_sim {
     // all-pairs partial forces: [nsplit][3][N] doubles
     double *fpart;
     int ap_nsplit;                // j splits of the general kernel
-    // all-pairs tiled kernel: spatial tiles ta x tb x tc, j splits, validity bound
+    // all-pairs tiled kernel: R atoms per thread, i blocks, j splits, Morton sort grid,
+    // pre-shift validity bound
     bool ap_tiled, ap_force_general;
-    int ap_ta, ap_tb, ap_tc, ap_ntiles, ap_tsplit, ap_since_sort;
+    int ap_R, ap_ntiles, ap_tsplit, ap_since_sort, ap_sort_g, ap_sort_bins;
     float ap_hmax;
     int *tile_count, *tile_start;
     // energy partials and results
@@ -108,6 +109,8 @@ int ljmd_ke_only(md_sim *s);
 int ljmd_reduce_energies(md_sim *s);
 int ljmd_forces_allpairs(md_sim *s);
 void ljmd_ap_plan(md_sim *s);
+void ljmd_ap_set_R(md_sim *s, int R);                       // R in {0 (general kernel), 1, 2, 4, 8}
+void ljmd_ap_caps(md_sim *s, int *max_split, int *max_blocks);
 int ljmd_scan_counts(md_sim *s, int *count, int *start, int n);   // exclusive scan, zeroes count
 int ljmd_cell_build(md_sim *s);
 int ljmd_forces_cell(md_sim *s);

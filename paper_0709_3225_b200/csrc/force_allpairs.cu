@@ -1,25 +1,32 @@
 // All-pairs O(N^2) Lennard-Jones force under minimum image.
 // PAPER.md:49-52 (Eq. 1) and :70-76 (Sec. 2.1): one thread per atom i, the j atoms staged
-// through shared memory in tiles shared by the block.  What differs from the paper's G80
-// kernel:
-//   * the inner loop is an FP32 distance FILTER: only ~0.16 % of pairs are inside rc at
-//     N = 32000, so the pair term is evaluated (exactly, in FP64, from the original
-//     coordinates) only for the few pairs the filter accepts;
-//   * atoms are sorted into spatial tiles; a block owns one tile and stages every j tile
-//     already shifted to the periodic image nearest the block's centre, so the minimum image
-//     disappears from the inner loop, and r^2 - |u_i|^2 = |u_j|^2 - 2 u_i.u_j costs 3 FFMA;
+// through shared memory in tiles shared by the block.  Every one of the N^2 ordered pair
+// distances is computed; what differs from the paper's G80 kernel:
+//   * the inner loop is an FP32 distance FILTER in 3 FFMA per pair: atoms are sorted along a
+//     Hilbert curve, a block owns 128 R consecutive atoms, and every chunk of 32 j atoms is
+//     staged (per warp, no block barrier) already shifted to the periodic image nearest the
+//     block's centre c, so the minimum image leaves the inner loop and
+//     r^2 - |u_i|^2 = |u_j|^2 - 2 u_i.u_j  (u = x - c);
+//   * the cutoff test is folded into a running minimum (one FMNMX3 per two pairs); only a
+//     32-j chunk whose minimum drops below the threshold is rescanned into hit masks;
+//   * hits (0.16 % of the pairs at N = 32000) go to a per-lane queue in shared memory and are
+//     drained in lockstep: the pair term is evaluated in FP64 from the stored coordinates,
+//     exactly as the oracle sees them, so the filter only has to be conservative;
 //   * each thread carries R atoms i in registers (one shared-memory load feeds 3R FFMA);
-//   * the j range is split across blockIdx.y so that small N still fills 148 SMs, and the
-//     partial forces are combined in a deterministic second pass.
+//   * the j chunks are dealt round-robin to blockIdx.y so that 148 SMs x 4 blocks are busy
+//     and the dense (nearby) chunks are spread evenly; the partial forces are combined in a
+//     deterministic second pass.
 // k_force_allpairs_general is the unsorted per-pair-minimum-image variant for boxes too small
-// to tile (L < ~4 rc) and the reference the tiled kernel is tested against.
+// to pre-shift (L/2 - rc smaller than a block) and the cross-check of the tiled kernel.
 #include <math.h>
 #include "common.cuh"
 #include "pair.cuh"
 
 #define AP_T 128      // threads per block
-#define AP_TJ 256     // j atoms staged per shared-memory tile
-#define AP_RMAX 6     // atoms i per thread, at most
+#define AP_TJ 32      // j atoms per staged chunk: one per lane
+#define AP_QCAP 48    // per-lane hit queue capacity (entries)
+#define AP_JBITS 27   // queue entry = r << 27 | j
+#define FULLMASK 0xffffffffu
 
 // ---------------------------------------------------------------------------------------
 // General variant: per-pair minimum image, valid for any rc <= L/2 and any atom order.
@@ -80,32 +87,61 @@ k_force_allpairs_general(const float4 *__restrict__ pos, int N, PairParams P, fl
 }
 
 // ---------------------------------------------------------------------------------------
-// Tile sort: counting sort of the state by spatial tile (ta x tb x tc uniform boxes).
-struct TileGrid { int a, b, c; float sa, sb, sc; };   // s* = count / L
+// Spatial sort: counting sort of the state by the Hilbert index of a cell on a 2^b grid
+// (side L / 2^b in [1.5, 3) sigma), so that any run of consecutive atoms is spatially compact
+// (a Hilbert curve has no jumps, unlike Morton order).
+struct SortGrid { int bits; float scale; };   // 2^bits cells per dimension, scale = 2^bits / L
+
+// Hilbert index of cell (x, y, z) on a 2^b cube: Skilling's axes-to-transpose transform
+// (AIP Conf. Proc. 707, 381 (2004)) followed by bit interleaving.
+__device__ __forceinline__ unsigned hilbert3(unsigned x, unsigned y, unsigned z, int b)
+{
+    unsigned X[3] = {x, y, z};
+    const unsigned M = 1u << (b - 1);
+    for (unsigned Q = M; Q > 1; Q >>= 1) {
+        const unsigned P = Q - 1;
+#pragma unroll
+        for (int i = 0; i < 3; i++) {
+            if (X[i] & Q) X[0] ^= P;
+            else { unsigned t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
+        }
+    }
+    X[1] ^= X[0];
+    X[2] ^= X[1];
+    unsigned t = 0;
+    for (unsigned Q = M; Q > 1; Q >>= 1)
+        if (X[2] & Q) t ^= Q - 1;
+    X[0] ^= t; X[1] ^= t; X[2] ^= t;
+    unsigned h = 0;
+    for (int k = b - 1; k >= 0; k--)
+        h = (h << 3) | (((X[0] >> k) & 1u) << 2) | (((X[1] >> k) & 1u) << 1) | ((X[2] >> k) & 1u);
+    return h;
+}
 
 __global__ void __launch_bounds__(256)
-k_bin_tile(const float4 *__restrict__ pos, int N, TileGrid g, int *__restrict__ tile_of, int *__restrict__ rank,
-           int *__restrict__ count)
+k_bin_hilbert(const float4 *__restrict__ pos, int N, SortGrid g, int *__restrict__ bin_of, int *__restrict__ rank,
+              int *__restrict__ count)
 {
     int i = blockIdx.x * 256 + threadIdx.x;
     if (i >= N) return;
     float4 p = pos[i];
-    int tx = min(g.a - 1, (int)(p.x * g.sa));
-    int ty = min(g.b - 1, (int)(p.y * g.sb));
-    int tz = min(g.c - 1, (int)(p.z * g.sc));
-    int t = (tx * g.b + ty) * g.c + tz;
-    tile_of[i] = t;
-    rank[i] = atomicAdd(&count[t], 1);
+    const int n = 1 << g.bits;
+    unsigned cx = min(n - 1, (int)(p.x * g.scale));
+    unsigned cy = min(n - 1, (int)(p.y * g.scale));
+    unsigned cz = min(n - 1, (int)(p.z * g.scale));
+    int b = (g.bits > 0) ? (int)hilbert3(cx, cy, cz, g.bits) : 0;
+    bin_of[i] = b;
+    rank[i] = atomicAdd(&count[b], 1);
 }
 
 __global__ void __launch_bounds__(256)
-k_scatter_tile(const float4 *__restrict__ pos, const float4 *__restrict__ vel, int N, const int *__restrict__ tile_of,
-               const int *__restrict__ rank, const int *__restrict__ start, float4 *__restrict__ pos2,
-               float4 *__restrict__ vel2)
+k_scatter_sorted(const float4 *__restrict__ pos, const float4 *__restrict__ vel, int N, const int *__restrict__ bin_of,
+                 const int *__restrict__ rank, const int *__restrict__ start, float4 *__restrict__ pos2,
+                 float4 *__restrict__ vel2)
 {
     int i = blockIdx.x * 256 + threadIdx.x;
     if (i >= N) return;
-    int dst = start[tile_of[i]] + rank[i];
+    int dst = start[bin_of[i]] + rank[i];
     pos2[dst] = pos[i];
     vel2[dst] = vel[i];
 }
@@ -124,45 +160,129 @@ __device__ __forceinline__ void ap_exact(const PairParams &P, const float4 &pi, 
     pair_f64(P, ex, ey, ez, fx, fy, fz, pe, w);
 }
 
-// One block = one tile of i atoms (R per thread) against the j range [jbeg, jend).
-template <int R>
-__device__ __forceinline__ void ap_sweep(const float4 *__restrict__ pos, int N, const PairParams &P, float L, float invL,
-                                         double Ld, double invLd, float hmax, int ibeg, int iend, int jbeg, int jend,
-                                         int split, double *__restrict__ fpart, double &pe, double &w,
-                                         float4 *tile, float *bb)
+// Drain this lane's hit queue: every lane evaluates its own entries, all lanes in lockstep,
+// two entries at a time (independent FP64 chains).
+// facc[(3 r + c) * AP_T + tid] is the FP64 force accumulator of this lane's atom r.
+__device__ __forceinline__ void ap_drain(const float4 *__restrict__ pos, int N, const PairParams &P, double Ld,
+                                         double invLd, const unsigned *q, int qn, int tid, int i0, double *facc,
+                                         double &pe, double &w)
 {
+    const unsigned JM = (1u << AP_JBITS) - 1u;
+    for (int n = 0; n < qn; n += 2) {
+        const unsigned e0 = q[n * AP_T + tid];
+        const bool two = n + 1 < qn;
+        const unsigned e1 = two ? q[(n + 1) * AP_T + tid] : e0;
+        const int r0 = (int)(e0 >> AP_JBITS), j0 = (int)(e0 & JM), r1 = (int)(e1 >> AP_JBITS), j1 = (int)(e1 & JM);
+        const int ia = i0 + r0 * 32, ib = i0 + r1 * 32;
+        const bool ok0 = j0 != ia && j0 < N, ok1 = two && j1 != ib && j1 < N;
+        const float4 pa = pos[ia], pb = pos[ib];
+        const float4 qa = pos[ok0 ? j0 : ia], qb = pos[ok1 ? j1 : ib];
+        double fx0 = 0.0, fy0 = 0.0, fz0 = 0.0, fx1 = 0.0, fy1 = 0.0, fz1 = 0.0, pe1 = 0.0, w1 = 0.0;
+        if (ok0) ap_exact(P, pa, qa, Ld, invLd, fx0, fy0, fz0, pe, w);
+        if (ok1) ap_exact(P, pb, qb, Ld, invLd, fx1, fy1, fz1, pe1, w1);
+        pe += pe1;
+        w += w1;
+        double *a = facc + (3 * r0) * AP_T + tid;
+        a[0] += fx0;
+        a[AP_T] += fy0;
+        a[2 * AP_T] += fz0;
+        double *b = facc + (3 * r1) * AP_T + tid;
+        b[0] += fx1;
+        b[AP_T] += fy1;
+        b[2 * AP_T] += fz1;
+    }
+}
+
+template <int R>
+__global__ void __launch_bounds__(AP_T, 4)
+k_force_allpairs_tiled(const float4 *__restrict__ pos, int N, PairParams P, float L, float invL, double Ld,
+                       double invLd, float hmax, int nchunks_j, double *__restrict__ fpart,
+                       double *__restrict__ part_pe, double *__restrict__ part_w)
+{
+    extern __shared__ __align__(16) unsigned char ap_smem[];
+    double *facc = (double *)ap_smem;                                   // [3 R][AP_T]
+    float4 *tile = (float4 *)(facc + 3 * R * AP_T);                     // [4 warps][2][AP_TJ]
+    unsigned *q = (unsigned *)(tile + (AP_T / 32) * 2 * AP_TJ);         // [AP_QCAP][AP_T]
+    float *bb = (float *)(q + AP_QCAP * AP_T);                          // [4 warps][12]
+    double *red = (double *)(bb + 48);                                  // [32]
+
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    int idx[R];
-    float4 xi[R];
+    const int split = blockIdx.y, nsplit = gridDim.y;
+    const int bbase = blockIdx.x * (AP_T * R);
+    const int i0 = bbase + wid * (32 * R) + lane;                        // atom r of this lane: i0 + 32 r
+
+#pragma unroll
+    for (int k = 0; k < 3 * R; k++) facc[k * AP_T + tid] = 0.0;
+
+    // ---- block geometry: periodic bounding box of the block's atoms.  Per dimension, a
+    // 32-bin occupancy mask locates the longest empty stretch of the circle [0,L); cutting the
+    // circle in its middle unwraps the coordinates, whatever images the atoms are stored as.
+    float ux[R], uy[R], uz[R];
+    unsigned occ[3] = {0u, 0u, 0u};
+    const float binscale = 32.f * invL;
+#pragma unroll
+    for (int r = 0; r < R; r++) {
+        const int i = i0 + 32 * r;
+        ux[r] = uy[r] = uz[r] = 0.f;
+        if (i < N) {
+            const float4 p = pos[i];
+            ux[r] = p.x; uy[r] = p.y; uz[r] = p.z;
+            occ[0] |= 1u << min(31, (int)(p.x * binscale));
+            occ[1] |= 1u << min(31, (int)(p.y * binscale));
+            occ[2] |= 1u << min(31, (int)(p.z * binscale));
+        }
+    }
+#pragma unroll
+    for (int d = 0; d < 3; d++) occ[d] = __reduce_or_sync(FULLMASK, occ[d]);
+    unsigned *bbu = (unsigned *)bb;
+    if (lane == 0) {
+#pragma unroll
+        for (int d = 0; d < 3; d++) bbu[wid * 3 + d] = occ[d];
+    }
+    __syncthreads();
+    float cut[3];
+    bool compact = true;
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        unsigned m = 0u;
+#pragma unroll
+        for (int k = 0; k < AP_T / 32; k++) m |= bbu[k * 3 + d];
+        unsigned e = ~m, last = e;
+        int len = 0;
+        while (e) {                                  // bit i of e: bins i .. i+len all empty (cyclic)
+            last = e;
+            e &= (e >> 1) | (e << 31);
+            len++;
+        }
+        if (len == 0) { compact = false; cut[d] = 0.f; }
+        else cut[d] = ((float)(__ffs(last) - 1) + 0.5f * (float)len) * (L * 0.03125f);
+    }
+    __syncthreads();
     float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
     for (int r = 0; r < R; r++) {
-        idx[r] = ibeg + tid + r * AP_T;
-        if (idx[r] < iend) {
-            xi[r] = pos[idx[r]];
-            mn[0] = fminf(mn[0], xi[r].x); mx[0] = fmaxf(mx[0], xi[r].x);
-            mn[1] = fminf(mn[1], xi[r].y); mx[1] = fmaxf(mx[1], xi[r].y);
-            mn[2] = fminf(mn[2], xi[r].z); mx[2] = fmaxf(mx[2], xi[r].z);
-        } else {
-            idx[r] = -1;
-            xi[r] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (i0 + 32 * r < N) {
+            float x = ux[r] - cut[0], y = uy[r] - cut[1], z = uz[r] - cut[2];
+            x += (x < 0.f) ? L : 0.f; y += (y < 0.f) ? L : 0.f; z += (z < 0.f) ? L : 0.f;
+            mn[0] = fminf(mn[0], x); mx[0] = fmaxf(mx[0], x);
+            mn[1] = fminf(mn[1], y); mx[1] = fmaxf(mx[1], y);
+            mn[2] = fminf(mn[2], z); mx[2] = fmaxf(mx[2], z);
         }
     }
-    // bounding box of the block's atoms -> centre c and half extent h
 #pragma unroll
     for (int d = 0; d < 3; d++) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
-            mn[d] = fminf(mn[d], __shfl_xor_sync(0xffffffffu, mn[d], o));
-            mx[d] = fmaxf(mx[d], __shfl_xor_sync(0xffffffffu, mx[d], o));
+            mn[d] = fminf(mn[d], __shfl_xor_sync(FULLMASK, mn[d], o));
+            mx[d] = fmaxf(mx[d], __shfl_xor_sync(FULLMASK, mx[d], o));
         }
     }
-    __syncthreads();
     if (lane == 0) {
 #pragma unroll
         for (int d = 0; d < 3; d++) { bb[wid * 6 + d] = mn[d]; bb[wid * 6 + 3 + d] = mx[d]; }
     }
     __syncthreads();
+    float cen[3], hm = 0.f;
 #pragma unroll
     for (int d = 0; d < 3; d++) {
         mn[d] = bb[d]; mx[d] = bb[3 + d];
@@ -171,13 +291,13 @@ __device__ __forceinline__ void ap_sweep(const float4 *__restrict__ pos, int N, 
             mn[d] = fminf(mn[d], bb[k * 6 + d]);
             mx[d] = fmaxf(mx[d], bb[k * 6 + 3 + d]);
         }
+        cen[d] = cut[d] + 0.5f * (mn[d] + mx[d]);
+        hm = fmaxf(hm, 0.5f * (mx[d] - mn[d]));
     }
-    const float cx = 0.5f * (mn[0] + mx[0]), cy = 0.5f * (mn[1] + mx[1]), cz = 0.5f * (mn[2] + mx[2]);
-    const float hx = 0.5f * (mx[0] - mn[0]), hy = 0.5f * (mx[1] - mn[1]), hz = 0.5f * (mx[2] - mn[2]);
-    const float hm = fmaxf(hx, fmaxf(hy, hz));
-    // every image chosen relative to c is the minimum image for pairs within rc iff
-    // h + rc <= L/2 (with slack); otherwise fall back to per-pair minimum image
-    const bool preshift = hm <= hmax;
+    // the image of j nearest the centre is the minimum image for every i of the block when
+    // half extent + rc <= L/2 (with slack); otherwise this block tests per-pair minimum images
+    const bool preshift = compact && hm <= hmax;
+    const float cx = cen[0], cy = cen[1], cz = cen[2];                  // block centre (any image)
 
     // filter threshold: rc^2 plus the rounding error of the 3-FFMA form at these magnitudes
     const float rcf = P.rcf;
@@ -185,136 +305,151 @@ __device__ __forceinline__ void ap_sweep(const float4 *__restrict__ pos, int N, 
     const float thr = (float)P.rc2 + 2e-6f * (M * M + 2.f * M * Mi) + 8.f * rcf * (L * 1.1920929e-7f) + 1e-6f * (float)P.rc2;
 
     float ax[R], ay[R], az[R], T[R];
-    double fx[R], fy[R], fz[R];
 #pragma unroll
     for (int r = 0; r < R; r++) {
-        float ux = xi[r].x - cx, uy = xi[r].y - cy, uz = xi[r].z - cz;
-        ax[r] = -2.f * ux; ay[r] = -2.f * uy; az[r] = -2.f * uz;
-        T[r] = (idx[r] >= 0) ? thr - fmaf(ux, ux, fmaf(uy, uy, uz * uz)) : -INFINITY;
-        fx[r] = fy[r] = fz[r] = 0.0;
+        float x = ux[r] - cx, y = uy[r] - cy, z = uz[r] - cz;
+        x = fmaf(-L, rintf(x * invL), x);
+        y = fmaf(-L, rintf(y * invL), y);
+        z = fmaf(-L, rintf(z * invL), z);
+        ax[r] = -2.f * x; ay[r] = -2.f * y; az[r] = -2.f * z;
+        T[r] = (i0 + 32 * r < N) ? thr - fmaf(x, x, fmaf(y, y, z * z)) : -INFINITY;
     }
 
-    for (int j0 = jbeg; j0 < jend; j0 += AP_TJ) {
-        __syncthreads();
-        for (int t = tid; t < AP_TJ; t += AP_T) {
-            int j = j0 + t;
-            float4 u = make_float4(0.f, 0.f, 0.f, INFINITY);       // padding never passes the filter
-            if (j < jend) {
-                float4 p = pos[j];
-                if (preshift) {
-                    u.x = p.x - cx; u.y = p.y - cy; u.z = p.z - cz;
-                    u.x = fmaf(-L, rintf(u.x * invL), u.x);
-                    u.y = fmaf(-L, rintf(u.y * invL), u.y);
-                    u.z = fmaf(-L, rintf(u.z * invL), u.z);
-                    u.w = fmaf(u.x, u.x, fmaf(u.y, u.y, u.z * u.z));
-                } else {
-                    u = make_float4(p.x, p.y, p.z, 0.f);
-                }
-            }
-            tile[t] = u;
+    // stage one chunk of 32 j atoms (per warp): u = image of x_j nearest the centre,
+    // w = |u|^2 (padding: w = +inf).  The global load of the next chunk is issued before the
+    // current one is processed, the shared-memory store after it.
+    auto chunk_load = [&](int jc) {
+        const int j = jc * AP_TJ + lane;
+        return (j < N) ? pos[j] : make_float4(0.f, 0.f, 0.f, INFINITY);
+    };
+    auto chunk_store = [&](float4 *dst, const float4 p) {
+        float4 u = make_float4(0.f, 0.f, 0.f, INFINITY);
+        if (p.w != INFINITY) {                      // pos.w carries an atom id: never +inf bits
+            u.x = p.x - cx; u.y = p.y - cy; u.z = p.z - cz;
+            u.x = fmaf(-L, rintf(u.x * invL), u.x);
+            u.y = fmaf(-L, rintf(u.y * invL), u.y);
+            u.z = fmaf(-L, rintf(u.z * invL), u.z);
+            u.w = fmaf(u.x, u.x, fmaf(u.y, u.y, u.z * u.z));
         }
-        __syncthreads();
-        const int ntile = min(AP_TJ, jend - j0);
-        if (preshift) {
-            for (int ch = 0; ch * 32 < ntile; ch++) {
-                const float4 *tj = tile + ch * 32;
-                bool any[R];
+        dst[lane] = u;
+    };
+
+    double pe = 0.0, w = 0.0;
+    int qn = 0;
+    int buf = 0;
+    float4 *wtile = tile + wid * (2 * AP_TJ);
+    if (split < nchunks_j) chunk_store(wtile, chunk_load(split));
+    __syncwarp();
+    for (int jc = split; jc < nchunks_j; jc += nsplit) {
+        const float4 *tc = wtile + buf * AP_TJ;
+        const int jn = jc + nsplit;
+        float4 pnext = make_float4(0.f, 0.f, 0.f, INFINITY);
+        if (jn < nchunks_j) pnext = chunk_load(jn);
+        do {
+            unsigned mask[R];
+            bool anyhit = false;
+            if (preshift) {
+                float m[R];
 #pragma unroll
-                for (int r = 0; r < R; r++) any[r] = false;
-#pragma unroll 8
-                for (int k = 0; k < 32; k++) {
-                    const float4 uj = tj[k];
+                for (int r = 0; r < R; r++) m[r] = INFINITY;
+#pragma unroll 4
+                for (int k = 0; k < 32; k += 2) {
+                    const float4 a = tc[k], b = tc[k + 1];
 #pragma unroll
                     for (int r = 0; r < R; r++) {
-                        float v = fmaf(ax[r], uj.x, fmaf(ay[r], uj.y, fmaf(az[r], uj.z, uj.w)));
-                        any[r] |= v < T[r];
+                        float v1 = fmaf(ax[r], a.x, fmaf(ay[r], a.y, fmaf(az[r], a.z, a.w)));
+                        float v2 = fmaf(ax[r], b.x, fmaf(ay[r], b.y, fmaf(az[r], b.z, b.w)));
+                        m[r] = fminf(m[r], fminf(v1, v2));
                     }
                 }
-                bool anyall = false;
+                bool hit = false;
 #pragma unroll
-                for (int r = 0; r < R; r++) anyall |= any[r];
-                if (__any_sync(0xffffffffu, anyall)) {
-                    // rare: some lane has a candidate inside rc in this chunk of 32 j's
+                for (int r = 0; r < R; r++) hit |= m[r] < T[r];
+                if (!__any_sync(FULLMASK, hit)) break;
+                // some pair of this chunk is inside the threshold: rescan into hit masks
 #pragma unroll
-                    for (int r = 0; r < R; r++) {
-                        if (!any[r]) continue;
-                        unsigned mask = 0;
+                for (int r = 0; r < R; r++) {
+                    mask[r] = 0u;
+                    if (__any_sync(FULLMASK, m[r] < T[r])) {
 #pragma unroll 4
                         for (int k = 0; k < 32; k++) {
-                            const float4 uj = tj[k];
-                            float v = fmaf(ax[r], uj.x, fmaf(ay[r], uj.y, fmaf(az[r], uj.z, uj.w)));
-                            mask |= (v < T[r]) ? (1u << k) : 0u;
+                            const float4 a = tc[k];
+                            float v = fmaf(ax[r], a.x, fmaf(ay[r], a.y, fmaf(az[r], a.z, a.w)));
+                            mask[r] |= (v < T[r]) ? (1u << k) : 0u;
                         }
-                        while (mask) {
-                            int k = __ffs(mask) - 1;
-                            mask &= mask - 1;
-                            int j = j0 + ch * 32 + k;
-                            if (j != idx[r]) ap_exact(P, xi[r], pos[j], Ld, invLd, fx[r], fy[r], fz[r], pe, w);
-                        }
+                        anyhit |= mask[r] != 0u;
                     }
                 }
-            }
-        } else {
-            // fallback for a block whose atoms are not compact: per-pair minimum image
+            } else {
+                // block not compact (atoms drifted across the box since the last sort): per-pair
+                // minimum image on the centred coordinates
 #pragma unroll
-            for (int r = 0; r < R; r++) {
-                if (idx[r] < 0) continue;
-                for (int k = 0; k < ntile; k++) {
-                    const float4 pj = tile[k];
-                    float dx = pj.x - xi[r].x, dy = pj.y - xi[r].y, dz = pj.z - xi[r].z;
-                    dx = fmaf(-L, rintf(dx * invL), dx);
-                    dy = fmaf(-L, rintf(dy * invL), dy);
-                    dz = fmaf(-L, rintf(dz * invL), dz);
-                    float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                    if (r2 < P.rc2f_filter && (j0 + k) != idx[r])
-                        ap_exact(P, xi[r], pj, Ld, invLd, fx[r], fy[r], fz[r], pe, w);
+                for (int r = 0; r < R; r++) {
+                    mask[r] = 0u;
+                    if (T[r] == -INFINITY) continue;
+                    for (int k = 0; k < 32; k++) {
+                        const float4 a = tc[k];
+                        float dx = fmaf(0.5f, ax[r], a.x), dy = fmaf(0.5f, ay[r], a.y), dz = fmaf(0.5f, az[r], a.z);
+                        dx = fmaf(-L, rintf(dx * invL), dx);
+                        dy = fmaf(-L, rintf(dy * invL), dy);
+                        dz = fmaf(-L, rintf(dz * invL), dz);
+                        float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                        mask[r] |= (r2 < thr && a.w != INFINITY) ? (1u << k) : 0u;
+                    }
+                    anyhit |= mask[r] != 0u;
                 }
             }
-        }
+            // push the hits on this lane's queue; drain whenever some lane's queue is full
+            const unsigned jbase = (unsigned)(jc * AP_TJ);
+            while (__any_sync(FULLMASK, anyhit)) {
+                anyhit = false;
+#pragma unroll
+                for (int r = 0; r < R; r++) {
+                    unsigned mk = mask[r];
+                    while (mk && qn < AP_QCAP) {
+                        const int k = __ffs(mk) - 1;
+                        mk &= mk - 1;
+                        q[qn * AP_T + tid] = ((unsigned)r << AP_JBITS) | (jbase + k);
+                        qn++;
+                    }
+                    mask[r] = mk;
+                    anyhit |= mk != 0u;
+                }
+                if (__any_sync(FULLMASK, anyhit)) {
+                    ap_drain(pos, N, P, Ld, invLd, q, qn, tid, i0, facc, pe, w);
+                    qn = 0;
+                }
+            }
+        } while (false);
+        if (jn < nchunks_j) chunk_store(wtile + (buf ^ 1) * AP_TJ, pnext);
+        __syncwarp();
+        buf ^= 1;
     }
+    ap_drain(pos, N, P, Ld, invLd, q, qn, tid, i0, facc, pe, w);
+
     const size_t base = (size_t)split * 3 * N;
 #pragma unroll
     for (int r = 0; r < R; r++) {
-        if (idx[r] >= 0) {
-            fpart[base + idx[r]] = fx[r];
-            fpart[base + (size_t)N + idx[r]] = fy[r];
-            fpart[base + 2 * (size_t)N + idx[r]] = fz[r];
-        }
-    }
-}
-
-__global__ void __launch_bounds__(AP_T)
-k_force_allpairs_tiled(const float4 *__restrict__ pos, const int *__restrict__ tile_start, int N, PairParams P,
-                       float L, float invL, double Ld, double invLd, float hmax, int jchunk,
-                       double *__restrict__ fpart, double *__restrict__ part_pe, double *__restrict__ part_w)
-{
-    __shared__ float4 tile[AP_TJ];
-    __shared__ float bb[(AP_T / 32) * 6];
-    __shared__ double red[32];
-    const int t = blockIdx.x, split = blockIdx.y;
-    const int tb = tile_start[t], te = tile_start[t + 1];
-    const int jbeg = split * jchunk, jend = min(N, jbeg + jchunk);
-    double pe = 0.0, w = 0.0;
-    // a tile larger than AP_T * AP_RMAX atoms takes several passes
-    for (int ibeg = tb; ibeg < te; ibeg += AP_T * AP_RMAX) {
-        const int iend = min(te, ibeg + AP_T * AP_RMAX);
-        const int R = (iend - ibeg + AP_T - 1) / AP_T;
-        switch (R) {
-        case 1: ap_sweep<1>(pos, N, P, L, invL, Ld, invLd, hmax, ibeg, iend, jbeg, jend, split, fpart, pe, w, tile, bb); break;
-        case 2: ap_sweep<2>(pos, N, P, L, invL, Ld, invLd, hmax, ibeg, iend, jbeg, jend, split, fpart, pe, w, tile, bb); break;
-        case 3: ap_sweep<3>(pos, N, P, L, invL, Ld, invLd, hmax, ibeg, iend, jbeg, jend, split, fpart, pe, w, tile, bb); break;
-        case 4: ap_sweep<4>(pos, N, P, L, invL, Ld, invLd, hmax, ibeg, iend, jbeg, jend, split, fpart, pe, w, tile, bb); break;
-        case 5: ap_sweep<5>(pos, N, P, L, invL, Ld, invLd, hmax, ibeg, iend, jbeg, jend, split, fpart, pe, w, tile, bb); break;
-        default: ap_sweep<6>(pos, N, P, L, invL, Ld, invLd, hmax, ibeg, iend, jbeg, jend, split, fpart, pe, w, tile, bb); break;
+        const int i = i0 + 32 * r;
+        if (i < N) {
+            fpart[base + i] = facc[(3 * r) * AP_T + tid];
+            fpart[base + (size_t)N + i] = facc[(3 * r + 1) * AP_T + tid];
+            fpart[base + 2 * (size_t)N + i] = facc[(3 * r + 2) * AP_T + tid];
         }
     }
     pe = block_sum(pe, red);
     w = block_sum(w, red);
-    if (threadIdx.x == 0) {
-        int b = split * gridDim.x + t;
+    if (tid == 0) {
+        const int b = split * gridDim.x + blockIdx.x;
         part_pe[b] = 0.5 * pe;
         part_w[b] = 0.5 * w;
     }
+}
+
+static size_t ap_smem_bytes(int R)
+{
+    return (size_t)3 * R * AP_T * sizeof(double) + (AP_T / 32) * 2 * AP_TJ * sizeof(float4) + (size_t)AP_QCAP * AP_T * sizeof(unsigned) +
+           48 * sizeof(float) + 32 * sizeof(double);
 }
 
 // Deterministic combine of the j-split partial forces: frc[i] = sum_s fpart[s][.][i].
@@ -334,70 +469,111 @@ k_combine_forces(float4 *__restrict__ frc, const double *__restrict__ fpart, int
 }
 
 // ---------------------------------------------------------------------------------------
-// Host side: choose the tile grid (md_create), sort, launch.
+// Host side: choose R and the j split (md_create), sort, launch.
+static int ap_sm_count()
+{
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+            sms <= 0)
+            sms = 148;
+    }
+    return sms;
+}
+
+// i blocks and j splits for R atoms per thread: one wave of 4 resident blocks per SM
+static void ap_shape(int64_t N, int R, int *iblocks, int *tsplit)
+{
+    const int ib = (int)((N + 128 * R - 1) / (128 * R));
+    const int ntj = (int)((N + AP_TJ - 1) / AP_TJ);
+    int k = (4 * ap_sm_count()) / ib;
+    if (k > ntj / 4) k = ntj / 4;                                   // at least 4 chunks per warp
+    if (k > 64) k = 64;
+    if (k < 1) k = 1;
+    *iblocks = ib;
+    *tsplit = k;
+}
+
+void ljmd_ap_set_R(md_sim *s, int R)
+{
+    s->ap_R = R;
+    s->ap_tiled = R > 0;
+    s->ap_ntiles = 0;
+    s->ap_tsplit = 1;
+    if (R > 0) ap_shape(s->N, R, &s->ap_ntiles, &s->ap_tsplit);
+}
+
+// Largest j split and block count over every R the tiled kernel can be asked to run with
+void ljmd_ap_caps(md_sim *s, int *max_split, int *max_blocks)
+{
+    *max_split = 1;
+    *max_blocks = 1;
+    for (int R = 1; R <= 8; R <<= 1) {
+        int ib, k;
+        ap_shape(s->N, R, &ib, &k);
+        if (k > *max_split) *max_split = k;
+        if (ib * k > *max_blocks) *max_blocks = ib * k;
+    }
+}
+
 void ljmd_ap_plan(md_sim *s)
 {
-    // tiles of ~480 atoms (R = 4 with 128 threads); every dimension needs >= amin tiles so
-    // that half a tile plus rc fits in L/2
     const double L = s->L, rc = s->rc;
     const double slack = 0.05 * rc;
     s->ap_hmax = (float)(0.5 * L - rc - slack);
-    s->ap_tiled = false;
-    s->ap_ntiles = 0;
-    double denom = L - 2.0 * (rc + slack) - 0.25;        // 0.25: atoms drift between re-sorts
-    if (denom <= 0) return;
-    int amin = (int)ceil(L / denom);
-    if (amin < 2) amin = 2;
-    const double target = 480.0;
-    double best = 1e300;
-    int ba = 0, bb = 0, bc = 0;
-    for (int a = amin; a <= 96; a++)
-        for (int b = a; b <= 96; b++)
-            for (int c = b; c <= 96; c++) {
-                double pop = (double)s->N / ((double)a * b * c);
-                if (pop < 100.0) break;
-                // prefer a population just below a multiple of AP_T (full register tiles)
-                double R = ceil((pop + 3.0 * sqrt(pop) * 0.5) / AP_T);
-                if (R > AP_RMAX) continue;
-                double waste = 1.0 - pop / (R * AP_T) + 0.02 * fabs(pop - target) / target + 0.01 * (c - a);
-                if (waste < best) { best = waste; ba = a; bb = b; bc = c; }
-            }
-    if (!ba) return;
-    s->ap_tiled = true;
-    s->ap_ta = ba; s->ap_tb = bb; s->ap_tc = bc;
-    s->ap_ntiles = ba * bb * bc;
-    // j splits: fill the GPU with resident blocks and balance them across the SMs
-    int sms = 148;
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
-    int maxsplit = (int)((s->N + 4 * AP_TJ - 1) / (4 * AP_TJ));     // at least 4 j tiles per block
-    if (maxsplit < 1) maxsplit = 1;
-    int bestsplit = 1;
-    double besteff = 0.0;
-    for (int k = 1; k <= maxsplit && k <= 64; k++) {
-        double blocks = (double)s->ap_ntiles * k;
-        double per_sm = blocks / sms;
-        if (per_sm > 5.0 && k > 1) break;                            // about 5 blocks resident per SM
-        double eff = per_sm / ceil(per_sm) * (per_sm >= 4.0 ? 1.0 : per_sm / 4.0);
-        if (eff > besteff + 1e-9) { besteff = eff; bestsplit = k; }
+    ljmd_ap_set_R(s, 0);
+    s->ap_sort_g = 0;
+    s->ap_sort_bins = 1;
+    if (s->N >= (1LL << AP_JBITS)) return;
+    // Hilbert grid: 2^b cells per dimension with side L / 2^b in [1.5, 3) sigma, b <= 6
+    int bits = 0;
+    while (bits < 6 && L / (double)(1 << (bits + 1)) >= 1.5) bits++;
+    s->ap_sort_g = bits;
+    s->ap_sort_bins = 1 << (3 * bits);
+    // largest R whose block of 128 R consecutive atoms (a cube of that volume, stretched by
+    // the Hilbert curve and the cell granularity) still fits the pre-shift bound; a block that
+    // turns out not to fit falls back to per-pair minimum images inside the kernel
+    const double vol_per_atom = L * L * L / (double)s->N;
+    for (int R = 8; R >= 1; R >>= 1) {
+        double side = cbrt(128.0 * R * vol_per_atom);
+        double h = 0.5 * side * 1.2 + 0.5 * L / (double)(1 << bits) + 0.3;   // 0.3: drift between re-sorts
+        if (h <= s->ap_hmax && s->N >= 128 * R) { ljmd_ap_set_R(s, R); break; }
     }
-    s->ap_tsplit = bestsplit;
 }
 
-static int ap_tile_sort(md_sim *s)
+static int ap_sort(md_sim *s)
 {
     int N = (int)s->N;
     int nb = (N + 255) / 256;
-    TileGrid g;
-    g.a = s->ap_ta; g.b = s->ap_tb; g.c = s->ap_tc;
-    g.sa = (float)(g.a / s->L); g.sb = (float)(g.b / s->L); g.sc = (float)(g.c / s->L);
-    k_bin_tile<<<nb, 256, 0, s->stream>>>(s->pos, N, g, s->cell_of, s->rank, s->tile_count);
+    SortGrid g;
+    g.bits = s->ap_sort_g;
+    g.scale = (float)((double)(1 << g.bits) / s->L);
+    k_bin_hilbert<<<nb, 256, 0, s->stream>>>(s->pos, N, g, s->cell_of, s->rank, s->tile_count);
     CKL(s);
-    int r = ljmd_scan_counts(s, s->tile_count, s->tile_start, s->ap_ntiles);
+    int r = ljmd_scan_counts(s, s->tile_count, s->tile_start, s->ap_sort_bins);
     if (r) return r;
-    k_scatter_tile<<<nb, 256, 0, s->stream>>>(s->pos, s->vel, N, s->cell_of, s->rank, s->tile_start, s->pos2, s->vel2);
+    k_scatter_sorted<<<nb, 256, 0, s->stream>>>(s->pos, s->vel, N, s->cell_of, s->rank, s->tile_start, s->pos2, s->vel2);
     CKL(s);
     float4 *t = s->pos; s->pos = s->pos2; s->pos2 = t;
     t = s->vel; s->vel = s->vel2; s->vel2 = t;
+    return MD_OK;
+}
+
+template <int R>
+static int ap_launch(md_sim *s, double *ppe, double *pw)
+{
+    static bool attr_set = false;
+    const size_t smem = ap_smem_bytes(R);
+    if (!attr_set) {
+        CK(cudaFuncSetAttribute(k_force_allpairs_tiled<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    const int N = (int)s->N;
+    dim3 grid(s->ap_ntiles, s->ap_tsplit);
+    k_force_allpairs_tiled<R><<<grid, AP_T, smem, s->stream>>>(s->pos, N, s->pp, s->Lf, 1.0f / s->Lf, s->L, 1.0 / s->L,
+                                                              s->ap_hmax, (N + AP_TJ - 1) / AP_TJ, s->fpart, ppe, pw);
+    CKL(s);
     return MD_OK;
 }
 
@@ -409,7 +585,7 @@ int ljmd_forces_allpairs(md_sim *s)
     int nsplit;
     if (s->ap_tiled && !s->ap_force_general) {
         if (s->layout != LAYOUT_TILE || s->ap_since_sort >= s->sort_every) {
-            int r = ap_tile_sort(s);
+            int r = ap_sort(s);
             if (r) return r;
             s->layout = LAYOUT_TILE;
             s->ap_since_sort = 0;
@@ -417,12 +593,14 @@ int ljmd_forces_allpairs(md_sim *s)
         }
         s->ap_since_sort++;
         nsplit = s->ap_tsplit;
-        int jchunk = (N + nsplit - 1) / nsplit;
-        jchunk = ((jchunk + AP_TJ - 1) / AP_TJ) * AP_TJ;
-        dim3 grid(s->ap_ntiles, nsplit);
-        k_force_allpairs_tiled<<<grid, AP_T, 0, s->stream>>>(s->pos, s->tile_start, N, s->pp, s->Lf, 1.0f / s->Lf,
-                                                            s->L, 1.0 / s->L, s->ap_hmax, jchunk, s->fpart, ppe, pw);
-        CKL(s);
+        int r;
+        switch (s->ap_R) {
+        case 8: r = ap_launch<8>(s, ppe, pw); break;
+        case 4: r = ap_launch<4>(s, ppe, pw); break;
+        case 2: r = ap_launch<2>(s, ppe, pw); break;
+        default: r = ap_launch<1>(s, ppe, pw); break;
+        }
+        if (r) return r;
         s->n_pe = s->ap_ntiles * nsplit;
     } else {
         int niblk = (N + AP_T - 1) / AP_T;

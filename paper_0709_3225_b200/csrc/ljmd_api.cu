@@ -211,8 +211,12 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->ap_nsplit = nsplit;
     ljmd_ap_plan(s);
     int cap_ap = niblk * nsplit;
-    if (s->ap_tiled && s->ap_ntiles * s->ap_tsplit > cap_ap) cap_ap = s->ap_ntiles * s->ap_tsplit;
-    if (s->ap_tiled && s->ap_tsplit > nsplit) nsplit = s->ap_tsplit;      // fpart holds either kernel's splits
+    {
+        int ms, mb;
+        ljmd_ap_caps(s, &ms, &mb);
+        if (mb > cap_ap) cap_ap = mb;
+        if (ms > nsplit) nsplit = ms;                                   // fpart holds either kernel's splits
+    }
     int cap_it = (int)((N + 255) / 256);
     s->part_cap = (cap_ap > cap_it ? cap_ap : cap_it) + 64;
 
@@ -234,7 +238,7 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->part = (double *)ljmd_dev_alloc((size_t)3 * s->part_cap * sizeof(double), st);
     s->energies = (double *)ljmd_dev_alloc(3 * sizeof(double), st);
     s->xfer = (float *)ljmd_dev_alloc((size_t)N * 3 * sizeof(float), st);
-    int ntiles = s->ap_tiled ? s->ap_ntiles : 1;
+    int ntiles = s->ap_sort_bins > 0 ? s->ap_sort_bins : 1;
     s->tile_count = (int *)ljmd_dev_alloc((size_t)ntiles * sizeof(int), st);
     s->tile_start = (int *)ljmd_dev_alloc(((size_t)ntiles + 1) * sizeof(int), st);
     if (!s->tile_count || !s->tile_start || !s->pos || !s->vel || !s->frc || !s->pos2 || !s->vel2 || !s->lpos || !s->cell_of || !s->rank ||
@@ -421,6 +425,12 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
         s->pp.precise_r2 = value;
     } else if (!strcmp(key, "ap_general")) {
         s->ap_force_general = value != 0.0;
+    } else if (!strcmp(key, "ap_R")) {
+        int R = (int)value;
+        if (R != 1 && R != 2 && R != 4 && R != 8) return MD_EINVAL;
+        if (s->N >= (1LL << 27)) return MD_EUNSUPPORTED;
+        ljmd_ap_set_R(s, R);
+        s->layout = LAYOUT_NONE;
     } else if (!strcmp(key, "sort_every")) {
         if (value < 1) return MD_EINVAL;
         s->sort_every = (int)value;
@@ -441,6 +451,7 @@ extern "C" int md_get_stat(md_sim *s, const char *key, double *value)
     else if (!strcmp(key, "ap_tiled")) *value = s->ap_tiled ? 1 : 0;
     else if (!strcmp(key, "ap_ntiles")) *value = s->ap_ntiles;
     else if (!strcmp(key, "ap_tsplit")) *value = s->ap_tsplit;
+    else if (!strcmp(key, "ap_R")) *value = s->ap_R;
     else if (!strcmp(key, "t_integrate_ms")) *value = s->t_phase[TAG_INTEGRATE];
     else if (!strcmp(key, "t_build_ms")) *value = s->t_phase[TAG_BUILD];
     else if (!strcmp(key, "t_force_ms")) *value = s->t_phase[TAG_FORCE];

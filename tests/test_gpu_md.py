@@ -59,13 +59,17 @@ def test_forces_cell_match_oracle(b, n, rho, amp, shifted):
 
 
 @pytest.mark.parametrize("n,rho,amp", [(7, 0.9, 0.08), (10, 0.8, 0.1), (12, 0.8, 0.1), (16, 0.5, 0.12)])
-def test_allpairs_tiled_kernel_is_used_and_matches_general(b, n, rho, amp):
-    """The tile-sorted, pre-shifted 3-FFMA filter kernel against the unsorted per-pair
-    minimum-image kernel and the oracle (several tiles, ragged R, several j splits)."""
+@pytest.mark.parametrize("R", [1, 2, 4, 8])
+def test_allpairs_sorted_kernel_matches_general_and_oracle(b, n, rho, amp, R):
+    """The Hilbert-sorted, pre-shifted 3-FFMA filter kernel (R atoms per thread) against the
+    unsorted per-pair minimum-image kernel and the oracle: ragged last block, several j
+    splits, and (large R in a small box) blocks too wide to pre-shift, which must fall back
+    to per-pair minimum images inside the kernel."""
     pos, L = wl.perturbed_fcc(n, rho, amp, seed=300 + n)
     vel = np.zeros_like(pos)
     with b.Sim(pos.shape[0], L) as s:
-        assert s.stat("ap_tiled") == 1 and s.stat("ap_ntiles") >= 8
+        s.option("ap_R", R)
+        assert s.stat("ap_tiled") == 1 and s.stat("ap_R") == R
         s.set_state(pos, vel)
         s.compute_forces(b.MD_ALLPAIRS)
         Ft, et = s.forces(), s.energies()
@@ -80,12 +84,22 @@ def test_allpairs_tiled_kernel_is_used_and_matches_general(b, n, rho, amp):
     assert et[1] == pytest.approx(peo, rel=1e-9) and et[2] == pytest.approx(wo, rel=1e-9)
 
 
+def test_allpairs_default_plan_uses_sorted_kernel_when_box_allows(b):
+    for n, want in ((5, 0), (10, 1), (20, 1)):
+        pos, L = wl.fcc_positions(n, 0.8)
+        with b.Sim(pos.shape[0], L) as s:
+            assert s.stat("ap_tiled") == want, n
+            if n == 20:
+                assert s.stat("ap_R") == 8
+
+
 def test_allpairs_tiled_after_drift_without_resort(b, oracle_uniforms):
     """Between re-sorts atoms leave their tile (and cross the periodic seam): the per-block
     bounding box check must keep the result exact."""
     pos, L = wl.fcc_positions(10, 0.8)
     vel = wl.maxwell_boltzmann(oracle_uniforms(wl.splitmix64(5) & wl.MASK48, 6 * 4000), 4000, 2.0)
     with b.Sim(4000, L) as s:
+        s.option("ap_R", 2)
         s.option("sort_every", 1000)
         s.set_state(pos, vel)
         s.step(300, b.MD_ALLPAIRS)
