@@ -9,9 +9,10 @@
 //     r^2 - |u_i|^2 = |u_j|^2 - 2 u_i.u_j  (u = x - c);
 //   * the cutoff test is folded into a running minimum (one FMNMX3 per two pairs); only a
 //     32-j chunk whose minimum drops below the threshold is rescanned into hit masks;
-//   * hits (0.16 % of the pairs at N = 32000) go to a per-lane queue in shared memory and are
-//     drained in lockstep: the pair term is evaluated in FP64 from the stored coordinates,
-//     exactly as the oracle sees them, so the filter only has to be conservative;
+//   * the hit masks (0.16 % of the pairs are hits at N = 32000) go to a per-lane queue in
+//     shared memory and are drained later, every lane walking its own hits: the pair term is
+//     evaluated in FP64 from the stored coordinates, exactly as the oracle sees them, so the
+//     filter only has to be conservative;
 //   * each thread carries R atoms i in registers (one shared-memory load feeds 3R FFMA);
 //   * the j chunks are dealt round-robin to blockIdx.y so that 148 SMs x 4 blocks are busy
 //     and the dense (nearby) chunks are spread evenly; the partial forces are combined in a
@@ -24,8 +25,8 @@
 
 #define AP_T 128      // threads per block
 #define AP_TJ 32      // j atoms per staged chunk: one per lane
-#define AP_QCAP 48    // per-lane hit queue capacity (entries)
-#define AP_JBITS 27   // queue entry = r << 27 | j
+#define AP_QCAP 24    // per-lane hit queue capacity (entries of 8 bytes: 32-bit hit mask, r and chunk base)
+#define AP_JBITS 27   // queue entry .y = r << 27 | first j of the chunk
 #define FULLMASK 0xffffffffu
 
 // ---------------------------------------------------------------------------------------
@@ -160,33 +161,39 @@ __device__ __forceinline__ void ap_exact(const PairParams &P, const float4 &pi, 
     pair_f64(P, ex, ey, ez, fx, fy, fz, pe, w);
 }
 
-// Drain this lane's hit queue: every lane evaluates its own entries, all lanes in lockstep,
-// two entries at a time (independent FP64 chains).
+// Drain this lane's hit queue.  An entry is the hit mask of one (atom r of this lane, chunk
+// of 32 j).  Every lane walks the hits of its own entries; even and odd entries form two
+// independent streams so that two FP64 pair evaluations are in flight per lane.
 // facc[(3 r + c) * AP_T + tid] is the FP64 force accumulator of this lane's atom r.
 __device__ __forceinline__ void ap_drain(const float4 *__restrict__ pos, int N, const PairParams &P, double Ld,
-                                         double invLd, const unsigned *q, int qn, int tid, int i0, double *facc,
+                                         double invLd, const uint2 *q, int qn, int tid, int i0, double *facc,
                                          double &pe, double &w)
 {
     const unsigned JM = (1u << AP_JBITS) - 1u;
-    for (int n = 0; n < qn; n += 2) {
-        const unsigned e0 = q[n * AP_T + tid];
-        const bool two = n + 1 < qn;
-        const unsigned e1 = two ? q[(n + 1) * AP_T + tid] : e0;
-        const int r0 = (int)(e0 >> AP_JBITS), j0 = (int)(e0 & JM), r1 = (int)(e1 >> AP_JBITS), j1 = (int)(e1 & JM);
-        const int ia = i0 + r0 * 32, ib = i0 + r1 * 32;
-        const bool ok0 = j0 != ia && j0 < N, ok1 = two && j1 != ib && j1 < N;
+    unsigned mka = 0u, mkb = 0u, infa = 0u, infb = 0u;
+    int na = 0, nb = 1;
+    for (;;) {
+        if (mka == 0u && na < qn) { const uint2 e = q[na * AP_T + tid]; mka = e.x; infa = e.y; na += 2; }
+        if (mkb == 0u && nb < qn) { const uint2 e = q[nb * AP_T + tid]; mkb = e.x; infb = e.y; nb += 2; }
+        if ((mka | mkb) == 0u) break;
+        const int ra = (int)(infa >> AP_JBITS), rb = (int)(infb >> AP_JBITS);
+        const int ia = i0 + ra * 32, ib = i0 + rb * 32;
+        int ja = ia, jb = ib;
+        if (mka) { ja = (int)(infa & JM) + __ffs(mka) - 1; mka &= mka - 1u; }
+        if (mkb) { jb = (int)(infb & JM) + __ffs(mkb) - 1; mkb &= mkb - 1u; }
+        const bool oka = ja != ia && ja < N, okb = jb != ib && jb < N;
         const float4 pa = pos[ia], pb = pos[ib];
-        const float4 qa = pos[ok0 ? j0 : ia], qb = pos[ok1 ? j1 : ib];
+        const float4 qa = pos[oka ? ja : ia], qb = pos[okb ? jb : ib];
         double fx0 = 0.0, fy0 = 0.0, fz0 = 0.0, fx1 = 0.0, fy1 = 0.0, fz1 = 0.0, pe1 = 0.0, w1 = 0.0;
-        if (ok0) ap_exact(P, pa, qa, Ld, invLd, fx0, fy0, fz0, pe, w);
-        if (ok1) ap_exact(P, pb, qb, Ld, invLd, fx1, fy1, fz1, pe1, w1);
+        if (oka) ap_exact(P, pa, qa, Ld, invLd, fx0, fy0, fz0, pe, w);
+        if (okb) ap_exact(P, pb, qb, Ld, invLd, fx1, fy1, fz1, pe1, w1);
         pe += pe1;
         w += w1;
-        double *a = facc + (3 * r0) * AP_T + tid;
+        double *a = facc + (3 * ra) * AP_T + tid;
         a[0] += fx0;
         a[AP_T] += fy0;
         a[2 * AP_T] += fz0;
-        double *b = facc + (3 * r1) * AP_T + tid;
+        double *b = facc + (3 * rb) * AP_T + tid;
         b[0] += fx1;
         b[AP_T] += fy1;
         b[2 * AP_T] += fz1;
@@ -202,7 +209,7 @@ k_force_allpairs_tiled(const float4 *__restrict__ pos, int N, PairParams P, floa
     extern __shared__ __align__(16) unsigned char ap_smem[];
     double *facc = (double *)ap_smem;                                   // [3 R][AP_T]
     float4 *tile = (float4 *)(facc + 3 * R * AP_T);                     // [4 warps][2][AP_TJ]
-    unsigned *q = (unsigned *)(tile + (AP_T / 32) * 2 * AP_TJ);         // [AP_QCAP][AP_T]
+    uint2 *q = (uint2 *)(tile + (AP_T / 32) * 2 * AP_TJ);               // [AP_QCAP][AP_T]
     float *bb = (float *)(q + AP_QCAP * AP_T);                          // [4 warps][12]
     double *red = (double *)(bb + 48);                                  // [32]
 
@@ -319,18 +326,16 @@ k_force_allpairs_tiled(const float4 *__restrict__ pos, int N, PairParams P, floa
     // w = |u|^2 (padding: w = +inf).  The global load of the next chunk is issued before the
     // current one is processed, the shared-memory store after it.
     auto chunk_load = [&](int jc) {
-        const int j = jc * AP_TJ + lane;
-        return (j < N) ? pos[j] : make_float4(0.f, 0.f, 0.f, INFINITY);
+        const int j = min(jc * AP_TJ + lane, N - 1);
+        return pos[j];
     };
-    auto chunk_store = [&](float4 *dst, const float4 p) {
-        float4 u = make_float4(0.f, 0.f, 0.f, INFINITY);
-        if (p.w != INFINITY) {                      // pos.w carries an atom id: never +inf bits
-            u.x = p.x - cx; u.y = p.y - cy; u.z = p.z - cz;
-            u.x = fmaf(-L, rintf(u.x * invL), u.x);
-            u.y = fmaf(-L, rintf(u.y * invL), u.y);
-            u.z = fmaf(-L, rintf(u.z * invL), u.z);
-            u.w = fmaf(u.x, u.x, fmaf(u.y, u.y, u.z * u.z));
-        }
+    auto chunk_store = [&](float4 *dst, const float4 p, bool valid) {
+        float4 u;
+        u.x = p.x - cx; u.y = p.y - cy; u.z = p.z - cz;
+        u.x = fmaf(-L, rintf(u.x * invL), u.x);
+        u.y = fmaf(-L, rintf(u.y * invL), u.y);
+        u.z = fmaf(-L, rintf(u.z * invL), u.z);
+        u.w = valid ? fmaf(u.x, u.x, fmaf(u.y, u.y, u.z * u.z)) : INFINITY;
         dst[lane] = u;
     };
 
@@ -338,16 +343,15 @@ k_force_allpairs_tiled(const float4 *__restrict__ pos, int N, PairParams P, floa
     int qn = 0;
     int buf = 0;
     float4 *wtile = tile + wid * (2 * AP_TJ);
-    if (split < nchunks_j) chunk_store(wtile, chunk_load(split));
+    if (split < nchunks_j) chunk_store(wtile, chunk_load(split), split * AP_TJ + lane < N);
     __syncwarp();
     for (int jc = split; jc < nchunks_j; jc += nsplit) {
         const float4 *tc = wtile + buf * AP_TJ;
         const int jn = jc + nsplit;
-        float4 pnext = make_float4(0.f, 0.f, 0.f, INFINITY);
-        if (jn < nchunks_j) pnext = chunk_load(jn);
+        const bool have_next = jn < nchunks_j;
+        float4 pnext = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (have_next) pnext = chunk_load(jn);
         do {
-            unsigned mask[R];
-            bool anyhit = false;
             if (preshift) {
                 float m[R];
 #pragma unroll
@@ -366,27 +370,41 @@ k_force_allpairs_tiled(const float4 *__restrict__ pos, int N, PairParams P, floa
 #pragma unroll
                 for (int r = 0; r < R; r++) hit |= m[r] < T[r];
                 if (!__any_sync(FULLMASK, hit)) break;
-                // some pair of this chunk is inside the threshold: rescan into hit masks
+                // some pair of this chunk is inside the threshold: rescan into hit masks.  A
+                // chunk adds at most R entries to a lane's queue: make room first.
+                if (__any_sync(FULLMASK, qn > AP_QCAP - R)) {
+                    ap_drain(pos, N, P, Ld, invLd, q, qn, tid, i0, facc, pe, w);
+                    qn = 0;
+                }
+                const unsigned jbase = (unsigned)(jc * AP_TJ);
 #pragma unroll
                 for (int r = 0; r < R; r++) {
-                    mask[r] = 0u;
                     if (__any_sync(FULLMASK, m[r] < T[r])) {
+                        unsigned mk = 0u;
 #pragma unroll 4
                         for (int k = 0; k < 32; k++) {
                             const float4 a = tc[k];
                             float v = fmaf(ax[r], a.x, fmaf(ay[r], a.y, fmaf(az[r], a.z, a.w)));
-                            mask[r] |= (v < T[r]) ? (1u << k) : 0u;
+                            mk |= (v < T[r]) ? (1u << k) : 0u;
                         }
-                        anyhit |= mask[r] != 0u;
+                        if (mk) {
+                            q[qn * AP_T + tid] = make_uint2(mk, ((unsigned)r << AP_JBITS) | jbase);
+                            qn++;
+                        }
                     }
                 }
             } else {
-                // block not compact (atoms drifted across the box since the last sort): per-pair
-                // minimum image on the centred coordinates
+                // block not compact (too wide for this box): per-pair minimum image on the
+                // centred coordinates
+                if (__any_sync(FULLMASK, qn > AP_QCAP - R)) {
+                    ap_drain(pos, N, P, Ld, invLd, q, qn, tid, i0, facc, pe, w);
+                    qn = 0;
+                }
+                const unsigned jbase = (unsigned)(jc * AP_TJ);
 #pragma unroll
                 for (int r = 0; r < R; r++) {
-                    mask[r] = 0u;
                     if (T[r] == -INFINITY) continue;
+                    unsigned mk = 0u;
                     for (int k = 0; k < 32; k++) {
                         const float4 a = tc[k];
                         float dx = fmaf(0.5f, ax[r], a.x), dy = fmaf(0.5f, ay[r], a.y), dz = fmaf(0.5f, az[r], a.z);
@@ -394,34 +412,16 @@ k_force_allpairs_tiled(const float4 *__restrict__ pos, int N, PairParams P, floa
                         dy = fmaf(-L, rintf(dy * invL), dy);
                         dz = fmaf(-L, rintf(dz * invL), dz);
                         float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                        mask[r] |= (r2 < thr && a.w != INFINITY) ? (1u << k) : 0u;
+                        mk |= (r2 < thr && a.w != INFINITY) ? (1u << k) : 0u;
                     }
-                    anyhit |= mask[r] != 0u;
-                }
-            }
-            // push the hits on this lane's queue; drain whenever some lane's queue is full
-            const unsigned jbase = (unsigned)(jc * AP_TJ);
-            while (__any_sync(FULLMASK, anyhit)) {
-                anyhit = false;
-#pragma unroll
-                for (int r = 0; r < R; r++) {
-                    unsigned mk = mask[r];
-                    while (mk && qn < AP_QCAP) {
-                        const int k = __ffs(mk) - 1;
-                        mk &= mk - 1;
-                        q[qn * AP_T + tid] = ((unsigned)r << AP_JBITS) | (jbase + k);
+                    if (mk) {
+                        q[qn * AP_T + tid] = make_uint2(mk, ((unsigned)r << AP_JBITS) | jbase);
                         qn++;
                     }
-                    mask[r] = mk;
-                    anyhit |= mk != 0u;
-                }
-                if (__any_sync(FULLMASK, anyhit)) {
-                    ap_drain(pos, N, P, Ld, invLd, q, qn, tid, i0, facc, pe, w);
-                    qn = 0;
                 }
             }
         } while (false);
-        if (jn < nchunks_j) chunk_store(wtile + (buf ^ 1) * AP_TJ, pnext);
+        if (have_next) chunk_store(wtile + (buf ^ 1) * AP_TJ, pnext, jn * AP_TJ + lane < N);
         __syncwarp();
         buf ^= 1;
     }
@@ -448,7 +448,7 @@ k_force_allpairs_tiled(const float4 *__restrict__ pos, int N, PairParams P, floa
 
 static size_t ap_smem_bytes(int R)
 {
-    return (size_t)3 * R * AP_T * sizeof(double) + (AP_T / 32) * 2 * AP_TJ * sizeof(float4) + (size_t)AP_QCAP * AP_T * sizeof(unsigned) +
+    return (size_t)3 * R * AP_T * sizeof(double) + (AP_T / 32) * 2 * AP_TJ * sizeof(float4) + (size_t)AP_QCAP * AP_T * sizeof(uint2) +
            48 * sizeof(float) + 32 * sizeof(double);
 }
 
