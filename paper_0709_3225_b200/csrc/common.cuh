@@ -42,6 +42,8 @@ struct Grid {
     float L;
 };
 
+enum { TAG_START = -1, TAG_INTEGRATE = 0, TAG_BUILD = 1, TAG_FORCE = 2, TAG_OTHER = 3, TAG_FORCE2 = 4, TAG_COUNT = 5 };
+
 struct md_sim {
     int64_t N;
     double L, rc, eps, sigma, dt;
@@ -70,6 +72,9 @@ struct md_sim {
     int ap_R, ap_ntiles, ap_tsplit, ap_since_sort, ap_sort_g, ap_sort_bins;
     float ap_hmax;
     int *tile_count, *tile_start;
+    // candidate lists of the sorted all-pairs kernel (allocated on first use)
+    int *nbr_count, *nbr_list;    // [N], [N][nbr_cap]
+    int nbr_cap;
     // energy partials and results
     double *part;                 // [3][part_cap] block partials: KE, PE, W
     int part_cap;
@@ -90,12 +95,11 @@ struct md_sim {
     cudaEvent_t *ev_pool;
     int *ev_tag;
     int ev_cap, ev_n;
-    double t_phase[4];            // ms: integrate, build, force kernel, other
-    int64_t n_phase[4];
+    double t_phase[TAG_COUNT];    // ms: integrate, build, force kernel, other, second force kernel
+    int64_t n_phase[TAG_COUNT];
 };
 
 enum { LAYOUT_NONE = 0, LAYOUT_CELL = 1, LAYOUT_TILE = 2 };
-enum { TAG_START = -1, TAG_INTEGRATE = 0, TAG_BUILD = 1, TAG_FORCE = 2, TAG_OTHER = 3 };
 // Record an event; the time since the previous tick is attributed to `tag`.
 void ljmd_tick(md_sim *s, int tag);
 int ljmd_collect_ticks(md_sim *s);
@@ -110,7 +114,6 @@ int ljmd_reduce_energies(md_sim *s);
 int ljmd_forces_allpairs(md_sim *s);
 void ljmd_ap_plan(md_sim *s);
 void ljmd_ap_set_R(md_sim *s, int R);                       // R in {0 (general kernel), 1, 2, 4, 8}
-void ljmd_ap_caps(md_sim *s, int *max_split, int *max_blocks);
 int ljmd_scan_counts(md_sim *s, int *count, int *start, int n);   // exclusive scan, zeroes count
 int ljmd_cell_build(md_sim *s);
 int ljmd_forces_cell(md_sim *s);

@@ -9,14 +9,15 @@
 //     r^2 - |u_i|^2 = |u_j|^2 - 2 u_i.u_j  (u = x - c);
 //   * the cutoff test is folded into a running minimum (one FMNMX3 per two pairs); only a
 //     32-j chunk whose minimum drops below the threshold is rescanned into hit masks;
-//   * the hit masks (0.16 % of the pairs are hits at N = 32000) go to a per-lane queue in
-//     shared memory and are drained later, every lane walking its own hits: the pair term is
-//     evaluated in FP64 from the stored coordinates, exactly as the oracle sees them, so the
-//     filter only has to be conservative;
+//   * the hits (0.16 % of the pairs at N = 32000) are appended to per-atom lists in global
+//     memory (one atomic per non-empty 32-pair mask), and a second kernel, one warp per atom,
+//     evaluates the listed pairs in FP64 from the stored coordinates, exactly as the oracle
+//     sees them, so the filter only has to be conservative and never holds a warp on an
+//     FP64 dependency chain; an atom with more hits than its list holds is rescanned against
+//     all j by its warp, so nothing is ever dropped;
 //   * each thread carries R atoms i in registers (one shared-memory load feeds 3R FFMA);
-//   * the j chunks are dealt round-robin to blockIdx.y so that 148 SMs x 4 blocks are busy
-//     and the dense (nearby) chunks are spread evenly; the partial forces are combined in a
-//     deterministic second pass.
+//   * the j chunks are dealt round-robin to blockIdx.y so that 148 SMs are busy and the dense
+//     (nearby) chunks are spread evenly.
 // k_force_allpairs_general is the unsorted per-pair-minimum-image variant for boxes too small
 // to pre-shift (L/2 - rc smaller than a block) and the cross-check of the tiled kernel.
 #include <math.h>
@@ -25,8 +26,8 @@
 
 #define AP_T 128      // threads per block
 #define AP_TJ 32      // j atoms per staged chunk: one per lane
-#define AP_QCAP 24    // per-lane hit queue capacity (entries of 8 bytes: 32-bit hit mask, r and chunk base)
-#define AP_JBITS 27   // queue entry .y = r << 27 | first j of the chunk
+#define AP_BPS 5      // resident filter blocks per SM (register bound, R = 8)
+#define AP_ET 256     // threads per block of the list evaluation kernel (32 atoms)
 #define FULLMASK 0xffffffffu
 
 // ---------------------------------------------------------------------------------------
@@ -161,65 +162,18 @@ __device__ __forceinline__ void ap_exact(const PairParams &P, const float4 &pi, 
     pair_f64(P, ex, ey, ez, fx, fy, fz, pe, w);
 }
 
-// Drain this lane's hit queue.  An entry is the hit mask of one (atom r of this lane, chunk
-// of 32 j).  Every lane walks the hits of its own entries; even and odd entries form two
-// independent streams so that two FP64 pair evaluations are in flight per lane.
-// facc[(3 r + c) * AP_T + tid] is the FP64 force accumulator of this lane's atom r.
-__device__ __forceinline__ void ap_drain(const float4 *__restrict__ pos, int N, const PairParams &P, double Ld,
-                                         double invLd, const uint2 *q, int qn, int tid, int i0, double *facc,
-                                         double &pe, double &w)
-{
-    const unsigned JM = (1u << AP_JBITS) - 1u;
-    unsigned mka = 0u, mkb = 0u, infa = 0u, infb = 0u;
-    int na = 0, nb = 1;
-    for (;;) {
-        if (mka == 0u && na < qn) { const uint2 e = q[na * AP_T + tid]; mka = e.x; infa = e.y; na += 2; }
-        if (mkb == 0u && nb < qn) { const uint2 e = q[nb * AP_T + tid]; mkb = e.x; infb = e.y; nb += 2; }
-        if ((mka | mkb) == 0u) break;
-        const int ra = (int)(infa >> AP_JBITS), rb = (int)(infb >> AP_JBITS);
-        const int ia = i0 + ra * 32, ib = i0 + rb * 32;
-        int ja = ia, jb = ib;
-        if (mka) { ja = (int)(infa & JM) + __ffs(mka) - 1; mka &= mka - 1u; }
-        if (mkb) { jb = (int)(infb & JM) + __ffs(mkb) - 1; mkb &= mkb - 1u; }
-        const bool oka = ja != ia && ja < N, okb = jb != ib && jb < N;
-        const float4 pa = pos[ia], pb = pos[ib];
-        const float4 qa = pos[oka ? ja : ia], qb = pos[okb ? jb : ib];
-        double fx0 = 0.0, fy0 = 0.0, fz0 = 0.0, fx1 = 0.0, fy1 = 0.0, fz1 = 0.0, pe1 = 0.0, w1 = 0.0;
-        if (oka) ap_exact(P, pa, qa, Ld, invLd, fx0, fy0, fz0, pe, w);
-        if (okb) ap_exact(P, pb, qb, Ld, invLd, fx1, fy1, fz1, pe1, w1);
-        pe += pe1;
-        w += w1;
-        double *a = facc + (3 * ra) * AP_T + tid;
-        a[0] += fx0;
-        a[AP_T] += fy0;
-        a[2 * AP_T] += fz0;
-        double *b = facc + (3 * rb) * AP_T + tid;
-        b[0] += fx1;
-        b[AP_T] += fy1;
-        b[2 * AP_T] += fz1;
-    }
-}
-
 template <int R>
-__global__ void __launch_bounds__(AP_T, 4)
-k_force_allpairs_tiled(const float4 *__restrict__ pos, int N, PairParams P, float L, float invL, double Ld,
-                       double invLd, float hmax, int nchunks_j, double *__restrict__ fpart,
-                       double *__restrict__ part_pe, double *__restrict__ part_w)
+__global__ void __launch_bounds__(AP_T, 5)
+k_allpairs_filter(const float4 *__restrict__ pos, int N, float rc, float rc2, float L, float invL, float hmax,
+                  int nchunks_j, int *__restrict__ nbr_count, int *__restrict__ nbr_list, int cap)
 {
-    extern __shared__ __align__(16) unsigned char ap_smem[];
-    double *facc = (double *)ap_smem;                                   // [3 R][AP_T]
-    float4 *tile = (float4 *)(facc + 3 * R * AP_T);                     // [4 warps][2][AP_TJ]
-    uint2 *q = (uint2 *)(tile + (AP_T / 32) * 2 * AP_TJ);               // [AP_QCAP][AP_T]
-    float *bb = (float *)(q + AP_QCAP * AP_T);                          // [4 warps][12]
-    double *red = (double *)(bb + 48);                                  // [32]
+    __shared__ float4 tile[(AP_T / 32) * 2 * AP_TJ];                    // [4 warps][2][AP_TJ]
+    __shared__ float bb[(AP_T / 32) * 6];
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int split = blockIdx.y, nsplit = gridDim.y;
     const int bbase = blockIdx.x * (AP_T * R);
     const int i0 = bbase + wid * (32 * R) + lane;                        // atom r of this lane: i0 + 32 r
-
-#pragma unroll
-    for (int k = 0; k < 3 * R; k++) facc[k * AP_T + tid] = 0.0;
 
     // ---- block geometry: periodic bounding box of the block's atoms.  Per dimension, a
     // 32-bin occupancy mask locates the longest empty stretch of the circle [0,L); cutting the
@@ -307,9 +261,9 @@ k_force_allpairs_tiled(const float4 *__restrict__ pos, int N, PairParams P, floa
     const float cx = cen[0], cy = cen[1], cz = cen[2];                  // block centre (any image)
 
     // filter threshold: rc^2 plus the rounding error of the 3-FFMA form at these magnitudes
-    const float rcf = P.rcf;
+    const float rcf = rc;
     const float Mi = 1.7320508f * hm, M = Mi + rcf;
-    const float thr = (float)P.rc2 + 2e-6f * (M * M + 2.f * M * Mi) + 8.f * rcf * (L * 1.1920929e-7f) + 1e-6f * (float)P.rc2;
+    const float thr = rc2 + 2e-6f * (M * M + 2.f * M * Mi) + 8.f * rcf * (L * 1.1920929e-7f) + 1e-6f * rc2;
 
     float ax[R], ay[R], az[R], T[R];
 #pragma unroll
@@ -339,8 +293,34 @@ k_force_allpairs_tiled(const float4 *__restrict__ pos, int N, PairParams P, floa
         dst[lane] = u;
     };
 
-    double pe = 0.0, w = 0.0;
-    int qn = 0;
+    // append the hits of one chunk to the lists of this lane's atoms: one atomic per non-empty
+    // mask reserves the slots (all R issued before any result is used), then the j indices
+    // are stored; slots beyond the capacity are counted but not stored (k_allpairs_eval then
+    // rescans that atom)
+    auto append = [&](unsigned (&mk)[R], int jbase) {
+        int base[R];
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            const int i = i0 + 32 * r;
+            const int self = i - jbase;                                 // the pair (i, i) is not a pair
+            if (self >= 0 && self < 32) mk[r] &= ~(1u << self);
+            base[r] = 0;
+            if (mk[r]) base[r] = atomicAdd(nbr_count + i, __popc(mk[r]));
+        }
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            unsigned m2 = mk[r];
+            int *row = nbr_list + (size_t)(i0 + 32 * r) * cap;
+            int b = base[r];
+            while (m2) {
+                const int k = __ffs(m2) - 1;
+                m2 &= m2 - 1u;
+                if (b < cap) row[b] = jbase + k;
+                b++;
+            }
+        }
+    };
+
     int buf = 0;
     float4 *wtile = tile + wid * (2 * AP_TJ);
     if (split < nchunks_j) chunk_store(wtile, chunk_load(split), split * AP_TJ + lane < N);
@@ -370,41 +350,31 @@ k_force_allpairs_tiled(const float4 *__restrict__ pos, int N, PairParams P, floa
 #pragma unroll
                 for (int r = 0; r < R; r++) hit |= m[r] < T[r];
                 if (!__any_sync(FULLMASK, hit)) break;
-                // some pair of this chunk is inside the threshold: rescan into hit masks.  A
-                // chunk adds at most R entries to a lane's queue: make room first.
-                if (__any_sync(FULLMASK, qn > AP_QCAP - R)) {
-                    ap_drain(pos, N, P, Ld, invLd, q, qn, tid, i0, facc, pe, w);
-                    qn = 0;
-                }
-                const unsigned jbase = (unsigned)(jc * AP_TJ);
+                // some pair of this chunk is inside the threshold: rescan into hit masks
+                const int jbase = jc * AP_TJ;
+                unsigned mk[R];
 #pragma unroll
                 for (int r = 0; r < R; r++) {
+                    mk[r] = 0u;
                     if (__any_sync(FULLMASK, m[r] < T[r])) {
-                        unsigned mk = 0u;
 #pragma unroll 4
                         for (int k = 0; k < 32; k++) {
                             const float4 a = tc[k];
                             float v = fmaf(ax[r], a.x, fmaf(ay[r], a.y, fmaf(az[r], a.z, a.w)));
-                            mk |= (v < T[r]) ? (1u << k) : 0u;
-                        }
-                        if (mk) {
-                            q[qn * AP_T + tid] = make_uint2(mk, ((unsigned)r << AP_JBITS) | jbase);
-                            qn++;
+                            mk[r] |= (v < T[r]) ? (1u << k) : 0u;
                         }
                     }
                 }
+                append(mk, jbase);
             } else {
                 // block not compact (too wide for this box): per-pair minimum image on the
                 // centred coordinates
-                if (__any_sync(FULLMASK, qn > AP_QCAP - R)) {
-                    ap_drain(pos, N, P, Ld, invLd, q, qn, tid, i0, facc, pe, w);
-                    qn = 0;
-                }
-                const unsigned jbase = (unsigned)(jc * AP_TJ);
+                const int jbase = jc * AP_TJ;
+                unsigned mk[R];
 #pragma unroll
                 for (int r = 0; r < R; r++) {
+                    mk[r] = 0u;
                     if (T[r] == -INFINITY) continue;
-                    unsigned mk = 0u;
                     for (int k = 0; k < 32; k++) {
                         const float4 a = tc[k];
                         float dx = fmaf(0.5f, ax[r], a.x), dy = fmaf(0.5f, ay[r], a.y), dz = fmaf(0.5f, az[r], a.z);
@@ -412,44 +382,68 @@ k_force_allpairs_tiled(const float4 *__restrict__ pos, int N, PairParams P, floa
                         dy = fmaf(-L, rintf(dy * invL), dy);
                         dz = fmaf(-L, rintf(dz * invL), dz);
                         float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                        mk |= (r2 < thr && a.w != INFINITY) ? (1u << k) : 0u;
-                    }
-                    if (mk) {
-                        q[qn * AP_T + tid] = make_uint2(mk, ((unsigned)r << AP_JBITS) | jbase);
-                        qn++;
+                        mk[r] |= (r2 < thr && a.w != INFINITY) ? (1u << k) : 0u;
                     }
                 }
+                append(mk, jbase);
             }
         } while (false);
         if (have_next) chunk_store(wtile + (buf ^ 1) * AP_TJ, pnext, jn * AP_TJ + lane < N);
         __syncwarp();
         buf ^= 1;
     }
-    ap_drain(pos, N, P, Ld, invLd, q, qn, tid, i0, facc, pe, w);
+}
 
-    const size_t base = (size_t)split * 3 * N;
-#pragma unroll
-    for (int r = 0; r < R; r++) {
-        const int i = i0 + 32 * r;
-        if (i < N) {
-            fpart[base + i] = facc[(3 * r) * AP_T + tid];
-            fpart[base + (size_t)N + i] = facc[(3 * r + 1) * AP_T + tid];
-            fpart[base + 2 * (size_t)N + i] = facc[(3 * r + 2) * AP_T + tid];
+// Eight lanes per atom: evaluate the listed candidate pairs in FP64 (Eq. 1-3)
+// from the stored coordinates, two independent chains per lane, reduce over the eight lanes,
+// write the force, reset the counter.
+#define AP_EL 8       // lanes per atom
+__global__ void __launch_bounds__(AP_ET)
+k_allpairs_eval(const float4 *__restrict__ pos, int N, PairParams P, double Ld, double invLd,
+                int *__restrict__ nbr_count, const int *__restrict__ nbr_list, int cap, float4 *__restrict__ frc,
+                double *__restrict__ part_pe, double *__restrict__ part_w)
+{
+    __shared__ double red[32];
+    const int sub = threadIdx.x & (AP_EL - 1);
+    const int i = blockIdx.x * (AP_ET / AP_EL) + (threadIdx.x / AP_EL);
+    double fx = 0.0, fy = 0.0, fz = 0.0, pe = 0.0, w = 0.0;
+    double gx = 0.0, gy = 0.0, gz = 0.0, pe2 = 0.0, w2 = 0.0;
+    if (i < N) {
+        const int n = nbr_count[i];
+        const float4 pi = pos[i];
+        if (n <= cap) {
+            const int *row = nbr_list + (size_t)i * cap;
+            int k = sub;
+            for (; k + AP_EL < n; k += 2 * AP_EL) {
+                const int ja = row[k], jb = row[k + AP_EL];
+                const float4 pa = pos[ja], pb = pos[jb];
+                ap_exact(P, pi, pa, Ld, invLd, fx, fy, fz, pe, w);
+                ap_exact(P, pi, pb, Ld, invLd, gx, gy, gz, pe2, w2);
+            }
+            if (k < n) ap_exact(P, pi, pos[row[k]], Ld, invLd, fx, fy, fz, pe, w);
+        } else {
+            // more candidates than the list holds: test every j (slow, never wrong)
+            for (int j = sub; j < N; j += AP_EL)
+                if (j != i) ap_exact(P, pi, pos[j], Ld, invLd, fx, fy, fz, pe, w);
         }
+    }
+    fx += gx; fy += gy; fz += gz; pe += pe2; w += w2;
+#pragma unroll
+    for (int o = AP_EL / 2; o > 0; o >>= 1) {
+        fx += __shfl_xor_sync(FULLMASK, fx, o);
+        fy += __shfl_xor_sync(FULLMASK, fy, o);
+        fz += __shfl_xor_sync(FULLMASK, fz, o);
+    }
+    if (i < N && sub == 0) {
+        frc[i] = make_float4((float)fx, (float)fy, (float)fz, 0.0f);
+        nbr_count[i] = 0;                           // ready for the next force evaluation
     }
     pe = block_sum(pe, red);
     w = block_sum(w, red);
-    if (tid == 0) {
-        const int b = split * gridDim.x + blockIdx.x;
-        part_pe[b] = 0.5 * pe;
-        part_w[b] = 0.5 * w;
+    if (threadIdx.x == 0) {
+        part_pe[blockIdx.x] = 0.5 * pe;             // every pair is visited from both ends
+        part_w[blockIdx.x] = 0.5 * w;
     }
-}
-
-static size_t ap_smem_bytes(int R)
-{
-    return (size_t)3 * R * AP_T * sizeof(double) + (AP_T / 32) * 2 * AP_TJ * sizeof(float4) + (size_t)AP_QCAP * AP_T * sizeof(uint2) +
-           48 * sizeof(float) + 32 * sizeof(double);
 }
 
 // Deterministic combine of the j-split partial forces: frc[i] = sum_s fpart[s][.][i].
@@ -482,12 +476,12 @@ static int ap_sm_count()
     return sms;
 }
 
-// i blocks and j splits for R atoms per thread: one wave of 4 resident blocks per SM
+// i blocks and j splits for R atoms per thread: one wave of AP_BPS resident blocks per SM
 static void ap_shape(int64_t N, int R, int *iblocks, int *tsplit)
 {
     const int ib = (int)((N + 128 * R - 1) / (128 * R));
     const int ntj = (int)((N + AP_TJ - 1) / AP_TJ);
-    int k = (4 * ap_sm_count()) / ib;
+    int k = (AP_BPS * ap_sm_count()) / ib;
     if (k > ntj / 4) k = ntj / 4;                                   // at least 4 chunks per warp
     if (k > 64) k = 64;
     if (k < 1) k = 1;
@@ -504,19 +498,6 @@ void ljmd_ap_set_R(md_sim *s, int R)
     if (R > 0) ap_shape(s->N, R, &s->ap_ntiles, &s->ap_tsplit);
 }
 
-// Largest j split and block count over every R the tiled kernel can be asked to run with
-void ljmd_ap_caps(md_sim *s, int *max_split, int *max_blocks)
-{
-    *max_split = 1;
-    *max_blocks = 1;
-    for (int R = 1; R <= 8; R <<= 1) {
-        int ib, k;
-        ap_shape(s->N, R, &ib, &k);
-        if (k > *max_split) *max_split = k;
-        if (ib * k > *max_blocks) *max_blocks = ib * k;
-    }
-}
-
 void ljmd_ap_plan(md_sim *s)
 {
     const double L = s->L, rc = s->rc;
@@ -525,7 +506,7 @@ void ljmd_ap_plan(md_sim *s)
     ljmd_ap_set_R(s, 0);
     s->ap_sort_g = 0;
     s->ap_sort_bins = 1;
-    if (s->N >= (1LL << AP_JBITS)) return;
+    if (s->N >= (1LL << 30)) return;
     // Hilbert grid: 2^b cells per dimension with side L / 2^b in [1.5, 3) sigma, b <= 6
     int bits = 0;
     while (bits < 6 && L / (double)(1 << (bits + 1)) >= 1.5) bits++;
@@ -561,19 +542,36 @@ static int ap_sort(md_sim *s)
 }
 
 template <int R>
-static int ap_launch(md_sim *s, double *ppe, double *pw)
+static int ap_launch(md_sim *s)
 {
-    static bool attr_set = false;
-    const size_t smem = ap_smem_bytes(R);
-    if (!attr_set) {
-        CK(cudaFuncSetAttribute(k_force_allpairs_tiled<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
     const int N = (int)s->N;
     dim3 grid(s->ap_ntiles, s->ap_tsplit);
-    k_force_allpairs_tiled<R><<<grid, AP_T, smem, s->stream>>>(s->pos, N, s->pp, s->Lf, 1.0f / s->Lf, s->L, 1.0 / s->L,
-                                                              s->ap_hmax, (N + AP_TJ - 1) / AP_TJ, s->fpart, ppe, pw);
+    k_allpairs_filter<R><<<grid, AP_T, 0, s->stream>>>(s->pos, N, (float)s->rc, (float)(s->rc * s->rc), s->Lf, 1.0f / s->Lf,
+                                                      s->ap_hmax, (N + AP_TJ - 1) / AP_TJ, s->nbr_count, s->nbr_list,
+                                                      s->nbr_cap);
     CKL(s);
+    return MD_OK;
+}
+
+// Candidate lists of the sorted kernel, allocated on first use: per atom, room for 2.5 times
+// the mean number of atoms inside rc (at least 64), a multiple of 32.
+static int ap_alloc_lists(md_sim *s)
+{
+    if (s->nbr_list) return MD_OK;
+    const double mean = 4.0 / 3.0 * 3.14159265358979 * s->rc * s->rc * s->rc * (double)s->N / (s->L * s->L * s->L);
+    int cap = (int)(2.5 * mean) + 32;
+    if (cap < 64) cap = 64;
+    cap = (cap + 31) / 32 * 32;
+    s->nbr_cap = cap;
+    s->nbr_count = (int *)ljmd_dev_alloc((size_t)s->N * sizeof(int), s->stream);
+    s->nbr_list = (int *)ljmd_dev_alloc((size_t)s->N * cap * sizeof(int), s->stream);
+    if (!s->nbr_count || !s->nbr_list) {
+        ljmd_dev_free(s->nbr_count, s->stream);
+        ljmd_dev_free(s->nbr_list, s->stream);
+        s->nbr_count = s->nbr_list = nullptr;
+        return MD_ENOMEM;
+    }
+    CK(cudaMemsetAsync(s->nbr_count, 0, (size_t)s->N * sizeof(int), s->stream));
     return MD_OK;
 }
 
@@ -582,29 +580,33 @@ int ljmd_forces_allpairs(md_sim *s)
     int N = (int)s->N;
     double *ppe = s->part + (size_t)s->part_cap;
     double *pw = s->part + 2 * (size_t)s->part_cap;
-    int nsplit;
     if (s->ap_tiled && !s->ap_force_general) {
+        int r = ap_alloc_lists(s);
+        if (r) return r;
         if (s->layout != LAYOUT_TILE || s->ap_since_sort >= s->sort_every) {
-            int r = ap_sort(s);
-            if (r) return r;
+            if ((r = ap_sort(s))) return r;
             s->layout = LAYOUT_TILE;
             s->ap_since_sort = 0;
             ljmd_tick(s, TAG_BUILD);
         }
         s->ap_since_sort++;
-        nsplit = s->ap_tsplit;
-        int r;
         switch (s->ap_R) {
-        case 8: r = ap_launch<8>(s, ppe, pw); break;
-        case 4: r = ap_launch<4>(s, ppe, pw); break;
-        case 2: r = ap_launch<2>(s, ppe, pw); break;
-        default: r = ap_launch<1>(s, ppe, pw); break;
+        case 8: r = ap_launch<8>(s); break;
+        case 4: r = ap_launch<4>(s); break;
+        case 2: r = ap_launch<2>(s); break;
+        default: r = ap_launch<1>(s); break;
         }
         if (r) return r;
-        s->n_pe = s->ap_ntiles * nsplit;
+        ljmd_tick(s, TAG_FORCE);
+        const int nb = (N + AP_ET / AP_EL - 1) / (AP_ET / AP_EL);
+        k_allpairs_eval<<<nb, AP_ET, 0, s->stream>>>(s->pos, N, s->pp, s->L, 1.0 / s->L, s->nbr_count, s->nbr_list,
+                                                    s->nbr_cap, s->frc, ppe, pw);
+        CKL(s);
+        s->n_pe = nb;
+        ljmd_tick(s, TAG_FORCE2);
     } else {
         int niblk = (N + AP_T - 1) / AP_T;
-        nsplit = s->ap_nsplit;
+        int nsplit = s->ap_nsplit;
         int jchunk = (N + nsplit - 1) / nsplit;
         jchunk = ((jchunk + AP_T - 1) / AP_T) * AP_T;
         dim3 grid(niblk, nsplit);
@@ -613,10 +615,10 @@ int ljmd_forces_allpairs(md_sim *s)
         CKL(s);
         s->n_pe = niblk * nsplit;
         if (s->layout == LAYOUT_CELL) s->layout = LAYOUT_NONE;      // lpos no longer tracked
+        ljmd_tick(s, TAG_FORCE);
+        k_combine_forces<<<(N + 255) / 256, 256, 0, s->stream>>>(s->frc, s->fpart, N, nsplit);
+        CKL(s);
+        ljmd_tick(s, TAG_OTHER);
     }
-    ljmd_tick(s, TAG_FORCE);
-    k_combine_forces<<<(N + 255) / 256, 256, 0, s->stream>>>(s->frc, s->fpart, N, nsplit);
-    CKL(s);
-    ljmd_tick(s, TAG_OTHER);
     return MD_OK;
 }

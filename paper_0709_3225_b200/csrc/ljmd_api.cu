@@ -166,7 +166,7 @@ static void free_all(md_sim *s)
     free(s->ev_pool);
     free(s->ev_tag);
     void *ptrs[] = {s->pos, s->vel, s->frc, s->pos2, s->vel2, s->lpos, s->cell_of, s->rank, s->cell_count,
-                    s->cell_start, s->max_occ, s->fpart, s->part, s->energies, s->xfer, s->tile_count,
+                    s->cell_start, s->max_occ, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list,
                     s->tile_start};
     for (void *p : ptrs) ljmd_dev_free(p, st);
 }
@@ -211,12 +211,7 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->ap_nsplit = nsplit;
     ljmd_ap_plan(s);
     int cap_ap = niblk * nsplit;
-    {
-        int ms, mb;
-        ljmd_ap_caps(s, &ms, &mb);
-        if (mb > cap_ap) cap_ap = mb;
-        if (ms > nsplit) nsplit = ms;                                   // fpart holds either kernel's splits
-    }
+    if ((int)((N + 7) / 8) > cap_ap) cap_ap = (int)((N + 7) / 8);       // k_allpairs_eval: 8 atoms per block
     int cap_it = (int)((N + 255) / 256);
     s->part_cap = (cap_ap > cap_it ? cap_ap : cap_it) + 64;
 
@@ -418,7 +413,7 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
     else if (!strcmp(key, "time_kernels")) {
         s->time_kernels = value != 0.0;
         s->ev_n = 0;
-        for (int k = 0; k < 4; k++) { s->t_phase[k] = 0.0; s->n_phase[k] = 0; }
+        for (int k = 0; k < TAG_COUNT; k++) { s->t_phase[k] = 0.0; s->n_phase[k] = 0; }
     }
     else if (!strcmp(key, "precise_r2")) {
         if (!(value >= 0)) return MD_EINVAL;
@@ -428,7 +423,6 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
     } else if (!strcmp(key, "ap_R")) {
         int R = (int)value;
         if (R != 1 && R != 2 && R != 4 && R != 8) return MD_EINVAL;
-        if (s->N >= (1LL << 27)) return MD_EUNSUPPORTED;
         ljmd_ap_set_R(s, R);
         s->layout = LAYOUT_NONE;
     } else if (!strcmp(key, "sort_every")) {
@@ -456,6 +450,8 @@ extern "C" int md_get_stat(md_sim *s, const char *key, double *value)
     else if (!strcmp(key, "t_build_ms")) *value = s->t_phase[TAG_BUILD];
     else if (!strcmp(key, "t_force_ms")) *value = s->t_phase[TAG_FORCE];
     else if (!strcmp(key, "t_other_ms")) *value = s->t_phase[TAG_OTHER];
+    else if (!strcmp(key, "t_force2_ms")) *value = s->t_phase[TAG_FORCE2];
+    else if (!strcmp(key, "nbr_cap")) *value = s->nbr_cap;
     else if (!strcmp(key, "n_force")) *value = (double)s->n_phase[TAG_FORCE];
     else if (!strcmp(key, "max_occupancy")) {
         int h = 0;
