@@ -1,13 +1,11 @@
-// Cell list: per-step build as a counting sort and the cell-list force
-// (row a4).  PAPER.md:98 (cells of side >= rc), :134 (n = int[L/rc]), :112 (27 neighbour
+// Cell list: per-step build as a counting sort; the force kernel (row a4)
+// is in force_cell.cu.  PAPER.md:98 (cells of side >= rc), :134 (n = int[L/rc]), :112 (27 neighbour
 // cells), :114-118 (the paper's serial per-cell append, replaced here by histogram + scan +
 // scatter).  Cells live on a power-of-two aligned grid so that cell-local coordinates and the
 // offsets between neighbouring cells are exact in FP32.
 #include "common.cuh"
-#include "pair.cuh"
 
 #define CB_T 256
-#define CF_T 128
 
 __device__ __forceinline__ int cell_coord(float x, const Grid &g)
 {
@@ -125,72 +123,5 @@ int ljmd_cell_build(md_sim *s)
     float4 *t = s->pos; s->pos = s->pos2; s->pos2 = t;
     t = s->vel; s->vel = s->vel2; s->vel2 = t;
     s->layout = LAYOUT_CELL;
-    return MD_OK;
-}
-
-// Cell-list force, full shell, one thread per atom in cell order.  The FP32 test on local
-// coordinates is a filter; accepted pairs are re-evaluated in FP64 from exact differences.
-__global__ void __launch_bounds__(CF_T)
-k_force_cell(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, int N, Grid g, PairParams P,
-             float4 *__restrict__ frc, double *__restrict__ part_pe, double *__restrict__ part_w)
-{
-    __shared__ double red[32];
-    const int i = blockIdx.x * CF_T + threadIdx.x;
-    double fx = 0.0, fy = 0.0, fz = 0.0, pe = 0.0, w = 0.0;
-    if (i < N) {
-        const float4 li = lpos[i];
-        const int c = __float_as_int(li.w);
-        const int n = g.n;
-        const int cz = c % n, cy = (c / n) % n, cx = c / (n * n);
-        for (int ax = -1; ax <= 1; ax++) {
-            int nx = cx + ax; nx += (nx < 0) ? n : 0; nx -= (nx >= n) ? n : 0;
-            float sx = (ax == 0) ? 0.f : (ax > 0 ? ((cx == n - 1) ? g.last : g.side)
-                                                 : -((nx == n - 1) ? g.last : g.side));
-            for (int ay = -1; ay <= 1; ay++) {
-                int ny = cy + ay; ny += (ny < 0) ? n : 0; ny -= (ny >= n) ? n : 0;
-                float sy = (ay == 0) ? 0.f : (ay > 0 ? ((cy == n - 1) ? g.last : g.side)
-                                                     : -((ny == n - 1) ? g.last : g.side));
-                for (int az = -1; az <= 1; az++) {
-                    int nz = cz + az; nz += (nz < 0) ? n : 0; nz -= (nz >= n) ? n : 0;
-                    float sz = (az == 0) ? 0.f : (az > 0 ? ((cz == n - 1) ? g.last : g.side)
-                                                         : -((nz == n - 1) ? g.last : g.side));
-                    const int nb = (nx * n + ny) * n + nz;
-                    const int jb = cell_start[nb], je = cell_start[nb + 1];
-                    // li relative to the neighbour cell's origin
-                    const float qx = li.x - sx, qy = li.y - sy, qz = li.z - sz;
-                    for (int j = jb; j < je; j++) {
-                        float4 pj = lpos[j];
-                        float dx = pj.x - qx, dy = pj.y - qy, dz = pj.z - qz;
-                        float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                        if (r2 < P.rc2f_filter && j != i) {
-                            double ex = ((double)pj.x - (double)li.x) + (double)sx;
-                            double ey = ((double)pj.y - (double)li.y) + (double)sy;
-                            double ez = ((double)pj.z - (double)li.z) + (double)sz;
-                            pair_f64(P, ex, ey, ez, fx, fy, fz, pe, w);
-                        }
-                    }
-                }
-            }
-        }
-        frc[i] = make_float4((float)fx, (float)fy, (float)fz, 0.0f);
-    }
-    pe = block_sum(pe, red);
-    w = block_sum(w, red);
-    if (threadIdx.x == 0) {
-        part_pe[blockIdx.x] = 0.5 * pe;
-        part_w[blockIdx.x] = 0.5 * w;
-    }
-}
-
-int ljmd_forces_cell(md_sim *s)
-{
-    int N = (int)s->N;
-    int nb = (N + CF_T - 1) / CF_T;
-    double *ppe = s->part + (size_t)s->part_cap;
-    double *pw = s->part + 2 * (size_t)s->part_cap;
-    k_force_cell<<<nb, CF_T, 0, s->stream>>>(s->lpos, s->cell_start, N, s->grid, s->pp, s->frc, ppe, pw);
-    CKL(s);
-    ljmd_tick(s, TAG_FORCE);
-    s->n_pe = nb;
     return MD_OK;
 }

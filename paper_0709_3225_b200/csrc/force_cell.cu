@@ -1,0 +1,304 @@
+// Cell-list Lennard-Jones force.  PAPER.md:112: one block (here: one
+// warp) per cell c0, the atoms of its 27 neighbour cells staged through shared memory.
+// What differs from the paper's G80 kernel (DESIGN.md sections 6, 7, 10):
+//   * CSR cells from the counting sort instead of 32 placeholders with virtual particles;
+//   * candidates are staged once per cell in the centre cell's frame, u = l + (offset between
+//     the two cell origins) - h, exact in FP32 on the power-of-two aligned grid;
+//   * the distance test is a FILTER, 3 FFMA + compare + ballot per (atom i, 32 candidates)
+//     row: lane = candidate (registers), the cell's atoms unrolled in registers,
+//     r^2 - |u_i|^2 = |u_j|^2 - 2 u_i.u_j against rc^2 + margin - |u_i|^2.  The ballot is the
+//     i-major hit-mask word, stored to shared memory;
+//   * evaluation: lane = (atom i, slice of its mask words); every lane walks its own hit bits,
+//     so only the 15 % of candidates inside rc reach the pair term and the lanes stay
+//     balanced (about 26 hits each at density 0.8);
+//   * mixed precision: pairs with r^2 < precise_r2 (default 1.3 sigma^2, the steep part of the
+//     potential) are queued and evaluated in FP64 from the exact local coordinates, the rest
+//     in FP32 with a Newton-corrected reciprocal; sums of s^6 and s^12 give PE and the virial.
+// Tiles over candidates (FC_CAP per pass) and over atoms (32 per pass): any occupancy works.
+#include <math.h>
+#include "common.cuh"
+#include "pair.cuh"
+
+#define FC_WARPS 4
+#define FC_T (FC_WARPS * 32)
+#define FC_CAP 512                    // staged candidates per pass
+#define FC_STEPS (FC_CAP / 32)
+#define FC_CLOSE 8                    // queued close pairs per lane and pass
+#define FULLMASK 0xffffffffu
+
+struct FcWarp {
+    float4 tile[FC_CAP];              // candidate in the centre cell's frame, w = |u|^2
+    unsigned msk[FC_STEPS][32];       // hit-mask words [32-candidate step][atom i of the pass]
+    unsigned short close[FC_CLOSE][32];
+    unsigned char kk[FC_CAP];         // neighbour cell (0..26) of each staged candidate
+    float4 seg[32];                   // per neighbour cell: origin offset minus h (x, y, z) and, as int
+                                      // bits, (first slot - candidates before the cell)
+    int seg_pref[32];                 // candidates before cell k; [27] = total
+};
+
+struct FcConst {
+    float rc2_lo, rc2_hi, p2, thr_margin, sig2, eps24, eps48, h;   // [rc2_lo, rc2_hi): decided in FP64
+    double hd;
+};
+
+__device__ __forceinline__ float fc_rcp(float x)      // 1/x, x normal and positive: MUFU + one Newton step
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    const float e = fmaf(-x, y, 1.f);
+    return fmaf(y, e, y);
+}
+
+// FP64 pair term of my atom (exact local coordinates lme) with staged candidate c of pass t0
+__device__ __forceinline__ void fc_precise(const FcWarp &S, const float4 *__restrict__ lpos, const PairParams &P,
+                                           const FcConst &K, const float4 &lme, int t0, int c, double &fx,
+                                           double &fy, double &fz, double &pe, double &w)
+{
+    const float4 sg = S.seg[S.kk[c]];
+    const float4 lj = lpos[__float_as_int(sg.w) + t0 + c];
+    const double ex = ((double)lj.x - (double)lme.x) + ((double)sg.x + K.hd);
+    const double ey = ((double)lj.y - (double)lme.y) + ((double)sg.y + K.hd);
+    const double ez = ((double)lj.z - (double)lme.z) + ((double)sg.z + K.hd);
+    pair_f64(P, ex, ey, ez, fx, fy, fz, pe, w);
+}
+
+// NI: atoms of the cell handled per pass (rows of the filter), 8 or 16.
+template <int NI, bool MODE2>
+__device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lpos, const int ibeg, const int ni,
+                                        const int total, const int mycnt, const PairParams &P, const FcConst &K,
+                                        float4 *__restrict__ frc, double &pe_tot, double &w_tot)
+{
+    const int lane = threadIdx.x & 31;
+    constexpr int G = NI, SL = 32 / NI;                 // lanes per slice, slices
+    const int li_ = lane & (G - 1), sl = lane / G;
+    const int cself0 = S.seg_pref[13];                  // candidate index of the cell's own atom 0
+    const int mypref = S.seg_pref[lane];
+    int staged_t0 = -1;
+
+    for (int i0 = 0; i0 < ni; i0 += NI) {
+        // rows of the filter: the pass's atoms, the same in every lane, two per FFMA2
+        float2 ax[NI / 2], ay[NI / 2], az[NI / 2];
+        float T[NI];
+#pragma unroll
+        for (int r = 0; r < NI; r++) {
+            const int idx = i0 + r;
+            const float4 l = lpos[ibeg + min(idx, ni - 1)];
+            const float x = l.x - K.h, y = l.y - K.h, z = l.z - K.h;
+            if (r & 1) { ax[r / 2].y = -2.f * x; ay[r / 2].y = -2.f * y; az[r / 2].y = -2.f * z; }
+            else { ax[r / 2].x = -2.f * x; ay[r / 2].x = -2.f * y; az[r / 2].x = -2.f * z; }
+            T[r] = (idx < ni) ? (K.rc2_hi + K.thr_margin) - fmaf(x, x, fmaf(y, y, z * z)) : -INFINITY;
+        }
+        // this lane's own atom in the evaluation phase
+        const int myidx = i0 + li_;
+        const bool myvalid = myidx < ni;
+        const float4 lme = lpos[ibeg + min(myidx, ni - 1)];
+        const float ux = lme.x - K.h, uy = lme.y - K.h, uz = lme.z - K.h;
+        float fx = 0.f, fy = 0.f, fz = 0.f, sA = 0.f, sB = 0.f, sR = 0.f;   // sums of s^12, s^6, (r - rc)
+        int nin = 0;
+        double dfx = 0.0, dfy = 0.0, dfz = 0.0, dpe = 0.0, dw = 0.0;
+
+        for (int t0 = 0; t0 < total; t0 += FC_CAP) {
+            const int cnt = min(FC_CAP, total - t0);
+            const int nsteps = (cnt + 31) >> 5;
+            if (t0 != staged_t0) {
+                // ---- stage the candidates t0 .. t0 + cnt of the concatenated neighbour cells
+                staged_t0 = t0;
+                __syncwarp();
+                {   // lane k < 27 labels the candidates of its cell
+                    const int lo = max(mypref, t0) - t0, hi = min(mypref + mycnt, t0 + cnt) - t0;
+                    for (int c = lo; c < hi; c++) S.kk[c] = (unsigned char)lane;
+                }
+                __syncwarp();
+                for (int c = lane; c < nsteps * 32; c += 32) {
+                    float4 u = make_float4(0.f, 0.f, 0.f, INFINITY);
+                    if (c < cnt) {
+                        const float4 sg = S.seg[S.kk[c]];
+                        const float4 l = lpos[__float_as_int(sg.w) + t0 + c];
+                        u.x = l.x + sg.x;
+                        u.y = l.y + sg.y;
+                        u.z = l.z + sg.z;
+                        u.w = fmaf(u.x, u.x, fmaf(u.y, u.y, u.z * u.z));
+                    }
+                    S.tile[c] = u;
+                }
+            }
+            __syncwarp();
+            // ---- filter: lane = candidate, rows = atoms
+            for (int st = 0; st < nsteps; st++) {
+                const float4 uj = S.tile[st * 32 + lane];
+                const float2 X = make_float2(uj.x, uj.x), Y = make_float2(uj.y, uj.y), Z = make_float2(uj.z, uj.z),
+                             W = make_float2(uj.w, uj.w);
+                unsigned word = 0u;
+#pragma unroll
+                for (int r = 0; r < NI / 2; r++) {
+                    const float2 v = __ffma2_rn(ax[r], X, __ffma2_rn(ay[r], Y, __ffma2_rn(az[r], Z, W)));
+                    const unsigned m0 = __ballot_sync(FULLMASK, v.x < T[2 * r]);
+                    const unsigned m1 = __ballot_sync(FULLMASK, v.y < T[2 * r + 1]);
+                    if (lane == 2 * r) word = m0;
+                    if (lane == 2 * r + 1) word = m1;
+                }
+                // the pair (i, i) is not a pair
+                const int cs = cself0 + i0 + lane - t0 - st * 32;
+                if (cs >= 0 && cs < 32) word &= ~(1u << cs);
+                S.msk[st][lane] = word;
+            }
+            __syncwarp();
+            // ---- evaluation: lane = (atom li_, slice sl), walking its own hit bits; the next
+            // mask word is fetched one word ahead
+            int ncl = 0;
+            int st = sl, stn = sl + SL;
+            unsigned cur = (myvalid && st < nsteps) ? S.msk[st][li_] : 0u;
+            bool more = myvalid && stn < nsteps;
+            unsigned nxt = more ? S.msk[stn][li_] : 0u;
+            for (;;) {
+                if (cur == 0u && more) {
+                    cur = nxt;
+                    st = stn;
+                    stn += SL;
+                    more = stn < nsteps;
+                    nxt = more ? S.msk[stn][li_] : 0u;
+                }
+                if (!__any_sync(FULLMASK, cur != 0u || more)) break;
+                if (cur) {
+                    const int b = 31 - __clz(cur);
+                    cur &= ~(1u << b);
+                    const int c = st * 32 + b;
+                    const float4 uj = S.tile[c];
+                    const float dx = uj.x - ux, dy = uj.y - uy, dz = uj.z - uz;
+                    const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                    // p2 <= r2 < rc2_lo: FP32 term.  r2 < p2 (steep part) and the sliver around
+                    // rc^2, where FP32 could misjudge the cutoff: FP64 from exact coordinates.
+                    const bool fast = r2 >= K.p2 && r2 < K.rc2_lo;
+                    if (!fast && r2 < K.rc2_hi) {
+                        if (ncl < FC_CLOSE) S.close[ncl++][lane] = (unsigned short)c;
+                        else fc_precise(S, lpos, P, K, lme, t0, c, dfx, dfy, dfz, dpe, dw);   // queue full
+                    }
+                    const float inv = fc_rcp(r2);
+                    const float s2 = K.sig2 * inv;
+                    float s6 = s2 * s2 * s2;
+                    s6 = fast ? s6 : 0.f;
+                    float fr = inv * s6 * fmaf(K.eps48, s6, -K.eps24);
+                    if (MODE2) {
+                        const float r = sqrtf(r2);
+                        fr -= fast ? P.f_rcf * inv * r : 0.f;
+                        sR += fast ? (r - P.rcf) : 0.f;
+                    }
+                    fx = fmaf(-fr, dx, fx);
+                    fy = fmaf(-fr, dy, fy);
+                    fz = fmaf(-fr, dz, fz);
+                    sA = fmaf(s6, s6, sA);
+                    sB += s6;
+                    nin += fast;
+                }
+            }
+            // ---- queued close pairs in FP64 from the exact local coordinates
+            const int maxcl = __reduce_max_sync(FULLMASK, ncl);
+            for (int q = 0; q < maxcl; q++)
+                if (q < ncl) fc_precise(S, lpos, P, K, lme, t0, (int)S.close[q][lane], dfx, dfy, dfz, dpe, dw);
+        }
+        // ---- combine the FP32 and FP64 parts, reduce over the slices, store
+        // PE = 4 eps (A - B) - n ushift [+ f_rc sum(r - rc)],  W = 24 eps (2A - B) [- f_rc sum r]
+        double tx = dfx + (double)fx, ty = dfy + (double)fy, tz = dfz + (double)fz;
+        double pe = dpe + P.eps4 * ((double)sA - (double)sB) - (double)nin * P.ushift;
+        double w = dw + P.eps24 * (2.0 * (double)sA - (double)sB);
+        if (MODE2) {
+            pe += P.f_rc * (double)sR;
+            w -= P.f_rc * ((double)sR + (double)nin * P.rc);
+        }
+#pragma unroll
+        for (int o = G; o < 32; o <<= 1) {
+            tx += __shfl_xor_sync(FULLMASK, tx, o);
+            ty += __shfl_xor_sync(FULLMASK, ty, o);
+            tz += __shfl_xor_sync(FULLMASK, tz, o);
+        }
+        if (myvalid && sl == 0) frc[ibeg + myidx] = make_float4((float)tx, (float)ty, (float)tz, 0.f);
+        pe_tot += pe;
+        w_tot += w;
+    }
+}
+
+template <bool MODE2>
+__global__ void __launch_bounds__(FC_T, 4)
+k_force_cell_warp(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, int ncells, Grid g,
+                  PairParams P, FcConst K, float4 *__restrict__ frc, double *__restrict__ part_pe,
+                  double *__restrict__ part_w)
+{
+    __shared__ FcWarp sm[FC_WARPS];
+    __shared__ double red[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int c = blockIdx.x * FC_WARPS + wid;
+    double pe = 0.0, w = 0.0;
+    if (c < ncells) {
+        const int ibeg = cell_start[c], ni = cell_start[c + 1] - ibeg;
+        if (ni > 0) {
+            FcWarp &S = sm[wid];
+            // the 27 neighbour cells, one per lane: slot range and origin offset
+            const int n = g.n;
+            const int cz = c % n, cy = (c / n) % n, cx = c / (n * n);
+            int cnt = 0, start = 0;
+            float ox = 0.f, oy = 0.f, oz = 0.f;
+            if (lane < 27) {
+                const int ax = lane / 9 - 1, ay = (lane / 3) % 3 - 1, az = lane % 3 - 1;
+                int nx = cx + ax, ny = cy + ay, nz = cz + az;
+                nx += (nx < 0) ? n : 0; nx -= (nx >= n) ? n : 0;
+                ny += (ny < 0) ? n : 0; ny -= (ny >= n) ? n : 0;
+                nz += (nz < 0) ? n : 0; nz -= (nz >= n) ? n : 0;
+                // distance between the two cell origins: exact
+                ox = (ax == 0) ? 0.f : (ax > 0 ? ((cx == n - 1) ? g.last : g.side) : -((nx == n - 1) ? g.last : g.side));
+                oy = (ay == 0) ? 0.f : (ay > 0 ? ((cy == n - 1) ? g.last : g.side) : -((ny == n - 1) ? g.last : g.side));
+                oz = (az == 0) ? 0.f : (az > 0 ? ((cz == n - 1) ? g.last : g.side) : -((nz == n - 1) ? g.last : g.side));
+                const int nb = (nx * n + ny) * n + nz;
+                start = cell_start[nb];
+                cnt = cell_start[nb + 1] - start;
+            }
+            int incl = cnt;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(FULLMASK, incl, o);
+                if (lane >= o) incl += y;
+            }
+            const int total = __shfl_sync(FULLMASK, incl, 31);
+            const int pref = incl - cnt;                 // lanes >= 27: total
+            S.seg_pref[lane] = pref;
+            S.seg[lane] = make_float4(ox - K.h, oy - K.h, oz - K.h, __int_as_float(start - pref));
+            __syncwarp();
+            if (ni <= 8) fc_cell<8, MODE2>(S, lpos, ibeg, ni, total, cnt, P, K, frc, pe, w);
+            else fc_cell<16, MODE2>(S, lpos, ibeg, ni, total, cnt, P, K, frc, pe, w);
+        }
+    }
+    pe = block_sum(pe, red);
+    w = block_sum(w, red);
+    if (threadIdx.x == 0) {
+        part_pe[blockIdx.x] = 0.5 * pe;              // every pair is visited from both ends
+        part_w[blockIdx.x] = 0.5 * w;
+    }
+}
+
+int ljmd_forces_cell(md_sim *s)
+{
+    const int ncells = s->grid.ncells;
+    const int nb = (ncells + FC_WARPS - 1) / FC_WARPS;
+    if (nb > s->part_cap) return MD_ENOMEM;
+    double *ppe = s->part + (size_t)s->part_cap;
+    double *pw = s->part + 2 * (size_t)s->part_cap;
+    const PairParams &P = s->pp;
+    FcConst K;
+    K.rc2_lo = (float)(P.rc2 * (1.0 - 4e-6));
+    K.rc2_hi = (float)(P.rc2 * (1.0 + 4e-6));
+    K.p2 = (float)fmin(P.precise_r2, 3.0e38);
+    K.h = 0.5f * s->grid.side;
+    K.hd = (double)K.h;
+    const double reach = 1.5 * (double)s->grid.last;
+    K.thr_margin = (float)(1e-5 * 3.0 * reach * reach + 1e-6 * P.rc2);
+    K.sig2 = P.sig2f;
+    K.eps24 = P.eps24f;
+    K.eps48 = 2.0f * P.eps24f;
+    if (P.mode == 2)
+        k_force_cell_warp<true><<<nb, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, ncells, s->grid, P, K, s->frc, ppe, pw);
+    else
+        k_force_cell_warp<false><<<nb, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, ncells, s->grid, P, K, s->frc, ppe, pw);
+    CKL(s);
+    ljmd_tick(s, TAG_FORCE);
+    s->n_pe = nb;
+    return MD_OK;
+}

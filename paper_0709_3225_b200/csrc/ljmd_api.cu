@@ -106,7 +106,7 @@ static void setup_pair(md_sim *s)
     P.ushift = (s->shifted >= 1) ? 4.0 * eps * (s6 * s6 - s6) : 0.0;
     P.f_rc = (s->shifted == 2) ? 24.0 * eps * (2.0 * s6 * s6 - s6) / rc : 0.0;
     P.mode = s->shifted;
-    P.precise_r2 = 1e300;
+    P.precise_r2 = 1.3 * sg * sg;       // cell path: FP64 below this r^2
     // FP32 filter threshold: rc^2 plus the worst-case rounding error of an FP32 r^2 computed
     // from box-scale coordinates (|d| error <= 2 ulp(L)), so the filter never rejects a pair
     // that is inside rc in exact arithmetic.
@@ -214,6 +214,7 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     if ((int)((N + 7) / 8) > cap_ap) cap_ap = (int)((N + 7) / 8);       // k_allpairs_eval: 8 atoms per block
     int cap_it = (int)((N + 255) / 256);
     s->part_cap = (cap_ap > cap_it ? cap_ap : cap_it) + 64;
+    if (s->grid.n && s->grid.ncells / 4 + 64 > s->part_cap) s->part_cap = s->grid.ncells / 4 + 64;   // one partial per 4 cells
 
     cudaStream_t st = s->stream;
     size_t f4 = (size_t)N * sizeof(float4);
