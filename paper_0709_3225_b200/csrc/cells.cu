@@ -29,55 +29,143 @@ k_bin(const float4 *__restrict__ pos, int N, Grid g, int *__restrict__ cell_of, 
     rank[i] = atomicAdd(&cell_count[c], 1);
 }
 
-// Exclusive scan of cell_count -> cell_start[0..ncells], max occupancy, and reset of the
-// counters for the next build.  One block; each thread owns a contiguous chunk.
-__global__ void __launch_bounds__(1024)
-k_scan_cells(int *__restrict__ cell_count, int *__restrict__ cell_start, int ncells, int *__restrict__ max_occ)
+// a1 + first half of a3 in one pass: [pending half-kick,] half-kick, drift, wrap, then the
+// histogram of the new position.  Same arithmetic as k_kick_drift (integrate.cu).
+template <int KICKS>
+__global__ void __launch_bounds__(CB_T)
+k_kick_drift_bin(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4 *__restrict__ frc, int N,
+                 float hdt, float dt, Grid g, int *__restrict__ cell_of, int *__restrict__ rank,
+                 int *__restrict__ cell_count)
 {
-    __shared__ int wsum[32];
-    __shared__ int wmax[32];
-    const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
-    const int chunk = (ncells + 1023) / 1024;
-    const int beg = min(ncells, t * chunk), end = min(ncells, beg + chunk);
-    int sum = 0, mx = 0;
-    for (int c = beg; c < end; c++) {
-        int v = cell_count[c];
-        sum += v;
-        mx = max(mx, v);
+    int i = blockIdx.x * CB_T + threadIdx.x;
+    if (i >= N) return;
+    float4 p = pos[i], v = vel[i];
+    const float4 f = frc[i];
+#pragma unroll
+    for (int k = 0; k < KICKS; k++) {
+        v.x = fmaf(hdt, f.x, v.x);
+        v.y = fmaf(hdt, f.y, v.y);
+        v.z = fmaf(hdt, f.z, v.z);
     }
+    p.x = wrap_drift(fmaf(dt, v.x, p.x), g.L);
+    p.y = wrap_drift(fmaf(dt, v.y, p.y), g.L);
+    p.z = wrap_drift(fmaf(dt, v.z, p.z), g.L);
+    pos[i] = p;
+    vel[i] = v;
+    int c = (cell_coord(p.x, g) * g.n + cell_coord(p.y, g)) * g.n + cell_coord(p.z, g);
+    cell_of[i] = c;
+    rank[i] = atomicAdd(&cell_count[c], 1);
+}
+
+// Exclusive scan of cell_count -> cell_start[0..ncells], max occupancy, and reset of the
+// counters for the next build.  Single pass over any number of cells: blocks take tiles of
+// SC_TILE cells in ticket order and chain their prefixes through `state` with a decoupled
+// look-back (one 64-bit word per tile: value | kind << 32 | epoch << 34, so words of earlier
+// launches read as "empty" and nothing has to be cleared between launches).
+#define SC_T 256
+#define SC_ITEMS 8
+#define SC_TILE (SC_T * SC_ITEMS)
+#define SC_AGG 1ull
+#define SC_PREFIX 2ull
+
+__device__ __forceinline__ unsigned long long sc_word(unsigned long long epoch, unsigned long long kind, int v)
+{
+    return (epoch << 34) | (kind << 32) | (unsigned)v;
+}
+
+__global__ void __launch_bounds__(SC_T)
+k_scan_cells(int *__restrict__ cell_count, int *__restrict__ cell_start, int ncells,
+             unsigned long long *__restrict__ max_occ,
+             unsigned *__restrict__ ticket, unsigned ticket_base, volatile unsigned long long *__restrict__ state,
+             unsigned long long epoch)
+{
+    __shared__ int wsum[SC_T / 32];
+    __shared__ int s_tile, s_prefix;
+    const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
+    if (t == 0) s_tile = (int)(atomicAdd(ticket, 1u) - ticket_base);
+    __syncthreads();
+    const int tile = s_tile;
+    const int base = tile * SC_TILE + t * SC_ITEMS;      // SC_ITEMS consecutive cells per thread
+    int v[SC_ITEMS];
+    int sum = 0, mx = 0;
+    if (base + SC_ITEMS <= ncells) {
+        const int4 a = *reinterpret_cast<const int4 *>(cell_count + base);
+        const int4 b = *reinterpret_cast<const int4 *>(cell_count + base + 4);
+        v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+    } else {
+#pragma unroll
+        for (int k = 0; k < SC_ITEMS; k++) v[k] = (base + k < ncells) ? cell_count[base + k] : 0;
+    }
+#pragma unroll
+    for (int k = 0; k < SC_ITEMS; k++) { sum += v[k]; mx = max(mx, v[k]); }
     int incl = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         int y = __shfl_up_sync(0xffffffffu, incl, o);
         if (lane >= o) incl += y;
     }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    mx = __reduce_max_sync(0xffffffffu, mx);
     if (lane == 31) wsum[wid] = incl;
-    if (lane == 0) wmax[wid] = mx;
+    // epoch-tagged maximum: a later launch always wins, so the word is never reset
+    if (lane == 0) atomicMax(max_occ, (epoch << 32) | (unsigned)mx);
     __syncthreads();
     if (wid == 0) {
-        int v = wsum[lane], m = wmax[lane];
-        int inc2 = v;
+        int ws = (lane < SC_T / 32) ? wsum[lane] : 0;
+        int inc2 = ws;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
+        for (int o = 1; o < SC_T / 32; o <<= 1) {
             int y = __shfl_up_sync(0xffffffffu, inc2, o);
             if (lane >= o) inc2 += y;
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
-        wsum[lane] = inc2 - v;                 // exclusive warp offsets
-        if (lane == 0) *max_occ = m;
+        const int agg = __shfl_sync(0xffffffffu, inc2, SC_T / 32 - 1);
+        if (lane < SC_T / 32) wsum[lane] = inc2 - ws;          // exclusive warp offsets
+        // publish the tile aggregate, then look back for the exclusive prefix
+        int prefix = 0;
+        if (tile == 0) {
+            if (lane == 0) state[0] = sc_word(epoch, SC_PREFIX, agg);
+        } else {
+            if (lane == 0) state[tile] = sc_word(epoch, SC_AGG, agg);
+            int look = tile - 1;
+            for (;;) {
+                const int idx = look - lane;
+                unsigned long long w = 0;
+                bool ready;
+                do {
+                    w = (idx >= 0) ? state[idx] : sc_word(epoch, SC_PREFIX, 0);
+                    ready = (w >> 34) == epoch && ((w >> 32) & 3ull) != 0ull;
+                } while (!__all_sync(0xffffffffu, ready));
+                const bool is_p = ((w >> 32) & 3ull) == SC_PREFIX;
+                const unsigned pm = __ballot_sync(0xffffffffu, is_p);
+                const int first_p = pm ? (__ffs(pm) - 1) : 32;          // nearest tile with a full prefix
+                int val = (lane <= first_p) ? (int)(unsigned)(w & 0xffffffffull) : 0;
+                prefix += __reduce_add_sync(0xffffffffu, val);
+                if (pm) break;
+                look -= 32;
+            }
+            if (lane == 0) {
+                __threadfence();
+                state[tile] = sc_word(epoch, SC_PREFIX, prefix + agg);
+            }
+        }
+        if (lane == 0) s_prefix = prefix;
     }
     __syncthreads();
-    int run = wsum[wid] + incl - sum;          // exclusive offset of this thread's chunk
-    for (int c = beg; c < end; c++) {
-        int v = cell_count[c];
-        cell_start[c] = run;
-        cell_count[c] = 0;
-        run += v;
+    int run = s_prefix + wsum[wid] + incl - sum;          // exclusive offset of this thread's first cell
+    int o[SC_ITEMS];
+#pragma unroll
+    for (int k = 0; k < SC_ITEMS; k++) { o[k] = run; run += v[k]; }
+    if (base + SC_ITEMS <= ncells) {
+        *reinterpret_cast<int4 *>(cell_start + base) = make_int4(o[0], o[1], o[2], o[3]);
+        *reinterpret_cast<int4 *>(cell_start + base + 4) = make_int4(o[4], o[5], o[6], o[7]);
+        *reinterpret_cast<int4 *>(cell_count + base) = make_int4(0, 0, 0, 0);
+        *reinterpret_cast<int4 *>(cell_count + base + 4) = make_int4(0, 0, 0, 0);
+        if (base + SC_ITEMS == ncells) cell_start[ncells] = run;
+    } else {
+#pragma unroll
+        for (int k = 0; k < SC_ITEMS; k++)
+            if (base + k < ncells) { cell_start[base + k] = o[k]; cell_count[base + k] = 0; }
+        if (base < ncells) cell_start[ncells] = run;      // the thread holding the last cell
     }
-    if (t == 1023) cell_start[ncells] = run;
 }
 
 // Scatter into cell order: state (global coordinates) and cell-local coordinates.
@@ -104,8 +192,28 @@ k_scatter(const float4 *__restrict__ pos, const float4 *__restrict__ vel, int N,
 
 int ljmd_scan_counts(md_sim *s, int *count, int *start, int n)
 {
-    k_scan_cells<<<1, 1024, 0, s->stream>>>(count, start, n, s->max_occ);
+    const int nb = (n + SC_TILE - 1) / SC_TILE;
+    if (nb > s->scan_cap) return MD_ENOMEM;
+    s->scan_epoch++;
+    k_scan_cells<<<nb, SC_T, 0, s->stream>>>(count, start, n, s->max_occ, s->scan_ticket, s->scan_ticket_base,
+                                             s->scan_state, (unsigned long long)(s->scan_epoch & 0x3fffffff));
+    s->scan_ticket_base += (unsigned)nb;
     CKL(s);
+    return MD_OK;
+}
+
+int ljmd_kick_drift_bin(md_sim *s, int kicks)
+{
+    int N = (int)s->N;
+    int nb = (N + CB_T - 1) / CB_T;
+    if (kicks == 2)
+        k_kick_drift_bin<2><<<nb, CB_T, 0, s->stream>>>(s->pos, s->vel, s->frc, N, s->hdtf, s->dtf, s->grid, s->cell_of,
+                                                        s->rank, s->cell_count);
+    else
+        k_kick_drift_bin<1><<<nb, CB_T, 0, s->stream>>>(s->pos, s->vel, s->frc, N, s->hdtf, s->dtf, s->grid, s->cell_of,
+                                                        s->rank, s->cell_count);
+    CKL(s);
+    s->binned = true;
     return MD_OK;
 }
 
@@ -113,8 +221,11 @@ int ljmd_cell_build(md_sim *s)
 {
     int N = (int)s->N;
     int nb = (N + CB_T - 1) / CB_T;
-    k_bin<<<nb, CB_T, 0, s->stream>>>(s->pos, N, s->grid, s->cell_of, s->rank, s->cell_count);
-    CKL(s);
+    if (!s->binned) {
+        k_bin<<<nb, CB_T, 0, s->stream>>>(s->pos, N, s->grid, s->cell_of, s->rank, s->cell_count);
+        CKL(s);
+    }
+    s->binned = false;
     int r = ljmd_scan_counts(s, s->cell_count, s->cell_start, s->grid.ncells);
     if (r) return r;
     k_scatter<<<nb, CB_T, 0, s->stream>>>(s->pos, s->vel, N, s->grid, s->cell_of, s->rank, s->cell_start,

@@ -62,7 +62,13 @@ struct md_sim {
     int *rank;                    // [N] rank inside its cell (during a build)
     int *cell_count;              // [ncells]
     int *cell_start;              // [ncells + 1]
-    int *max_occ;                 // [1]
+    unsigned long long *max_occ;  // [1] epoch << 32 | max cell occupancy of the last scan
+    // multi-block scan: ticket counter, per-tile look-back words, launch epoch
+    unsigned *scan_ticket;
+    unsigned scan_ticket_base;
+    unsigned long long *scan_state;
+    int scan_cap;
+    unsigned long long scan_epoch;
     // all-pairs partial forces: [nsplit][3][N] doubles
     double *fpart;
     int ap_nsplit;                // j splits of the general kernel
@@ -83,6 +89,7 @@ struct md_sim {
     float *xfer;                  // [N][3] staging for host/device packing
     int layout;                   // LAYOUT_*: how the slots are currently ordered
     bool has_state, forces_valid;
+    bool binned;                  // cell_of/rank/cell_count already hold the histogram of the current positions
     int forces_algo;
     bool use_graph;
     int sort_every;
@@ -107,7 +114,8 @@ int ljmd_collect_ticks(md_sim *s);
 // ---- kernels' host launchers (each returns md_status) ---------------------------
 int ljmd_pack_state(md_sim *s, const float *dpos, const float *dvel);
 int ljmd_unpack(md_sim *s, const float4 *src, float *dout);        // [N][3], caller's order
-int ljmd_kick_drift(md_sim *s);
+int ljmd_kick_drift(md_sim *s, int kicks);           // kicks = 2: plus the pending half-kick of the previous step
+int ljmd_kick_drift_bin(md_sim *s, int kicks);       // same, fused with the cell histogram
 int ljmd_kick_ke(md_sim *s);
 int ljmd_ke_only(md_sim *s);
 int ljmd_reduce_energies(md_sim *s);
@@ -119,6 +127,15 @@ int ljmd_cell_build(md_sim *s);
 int ljmd_forces_cell(md_sim *s);
 
 // ---- small device helpers --------------------------------------------------------
+// Wrap x into [0,L) after a drift of less than L (R14): a result that rounds to L becomes 0.
+__device__ __forceinline__ float wrap_drift(float x, float L)
+{
+    if (x >= L) x -= L;
+    else if (x < 0.0f) x += L;
+    if (x >= L || x < 0.0f) x = 0.0f;
+    return x;
+}
+
 __device__ __forceinline__ double warp_sum(double v)
 {
 #pragma unroll

@@ -28,7 +28,7 @@
 
 struct FcWarp {
     float4 tile[FC_CAP];              // candidate in the centre cell's frame, w = |u|^2
-    unsigned msk[FC_STEPS][32];       // hit-mask words [32-candidate step][atom i of the pass]
+    unsigned msk[FC_STEPS][16];       // hit-mask words [32-candidate step][atom i of the pass]
     unsigned short close[FC_CLOSE][32];
     unsigned char kk[FC_CAP];         // neighbour cell (0..26) of each staged candidate
     float4 seg[32];                   // per neighbour cell: origin offset minus h (x, y, z) and, as int
@@ -62,39 +62,27 @@ __device__ __forceinline__ void fc_precise(const FcWarp &S, const float4 *__rest
     pair_f64(P, ex, ey, ez, fx, fy, fz, pe, w);
 }
 
-// NI: atoms of the cell handled per pass (rows of the filter), 8 or 16.
+// NI: rows of the filter = atoms of the cell handled per pass (8 or 16).
 template <int NI, bool MODE2>
 __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lpos, const int ibeg, const int ni,
                                         const int total, const int mycnt, const PairParams &P, const FcConst &K,
                                         float4 *__restrict__ frc, double &pe_tot, double &w_tot)
 {
     const int lane = threadIdx.x & 31;
-    constexpr int G = NI, SL = 32 / NI;                 // lanes per slice, slices
-    const int li_ = lane & (G - 1), sl = lane / G;
     const int cself0 = S.seg_pref[13];                  // candidate index of the cell's own atom 0
     const int mypref = S.seg_pref[lane];
     int staged_t0 = -1;
 
     for (int i0 = 0; i0 < ni; i0 += NI) {
-        // rows of the filter: the pass's atoms, the same in every lane, two per FFMA2
-        float2 ax[NI / 2], ay[NI / 2], az[NI / 2];
-        float T[NI];
-#pragma unroll
-        for (int r = 0; r < NI; r++) {
-            const int idx = i0 + r;
-            const float4 l = lpos[ibeg + min(idx, ni - 1)];
-            const float x = l.x - K.h, y = l.y - K.h, z = l.z - K.h;
-            if (r & 1) { ax[r / 2].y = -2.f * x; ay[r / 2].y = -2.f * y; az[r / 2].y = -2.f * z; }
-            else { ax[r / 2].x = -2.f * x; ay[r / 2].x = -2.f * y; az[r / 2].x = -2.f * z; }
-            T[r] = (idx < ni) ? (K.rc2_hi + K.thr_margin) - fmaf(x, x, fmaf(y, y, z * z)) : -INFINITY;
-        }
-        // this lane's own atom in the evaluation phase
-        const int myidx = i0 + li_;
-        const bool myvalid = myidx < ni;
-        const float4 lme = lpos[ibeg + min(myidx, ni - 1)];
+        // evaluation mapping of this pass: nrow atoms, SL slices of the mask words per atom
+        const int nrow = min(NI, ni - i0);
+        const int SL = 32 / nrow;
+        const int sl = lane / nrow, li_ = lane - sl * nrow;
+        const bool myvalid = sl < SL;
+        const float4 lme = lpos[ibeg + i0 + li_];
         const float ux = lme.x - K.h, uy = lme.y - K.h, uz = lme.z - K.h;
         float fx = 0.f, fy = 0.f, fz = 0.f, sA = 0.f, sB = 0.f, sR = 0.f;   // sums of s^12, s^6, (r - rc)
-        int nin = 0;
+        int nhit = 0, nslow = 0;
         double dfx = 0.0, dfy = 0.0, dfz = 0.0, dpe = 0.0, dw = 0.0;
 
         for (int t0 = 0; t0 < total; t0 += FC_CAP) {
@@ -123,81 +111,103 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
                 }
             }
             __syncwarp();
-            // ---- filter: lane = candidate, rows = atoms
-            for (int st = 0; st < nsteps; st++) {
-                const float4 uj = S.tile[st * 32 + lane];
-                const float2 X = make_float2(uj.x, uj.x), Y = make_float2(uj.y, uj.y), Z = make_float2(uj.z, uj.z),
-                             W = make_float2(uj.w, uj.w);
-                unsigned word = 0u;
+            // ---- filter: lane = candidate, rows = atoms (two per FFMA2); the ballots of four rows
+            // go to shared memory as one 16-byte store (every lane writes the same value)
+            {
+                float2 ax[NI / 2], ay[NI / 2], az[NI / 2];
+                float T[NI];
 #pragma unroll
-                for (int r = 0; r < NI / 2; r++) {
-                    const float2 v = __ffma2_rn(ax[r], X, __ffma2_rn(ay[r], Y, __ffma2_rn(az[r], Z, W)));
-                    const unsigned m0 = __ballot_sync(FULLMASK, v.x < T[2 * r]);
-                    const unsigned m1 = __ballot_sync(FULLMASK, v.y < T[2 * r + 1]);
-                    if (lane == 2 * r) word = m0;
-                    if (lane == 2 * r + 1) word = m1;
+                for (int r = 0; r < NI; r++) {
+                    const int idx = i0 + r;
+                    const float4 l = lpos[ibeg + min(idx, ni - 1)];
+                    const float x = l.x - K.h, y = l.y - K.h, z = l.z - K.h;
+                    if (r & 1) { ax[r / 2].y = -2.f * x; ay[r / 2].y = -2.f * y; az[r / 2].y = -2.f * z; }
+                    else { ax[r / 2].x = -2.f * x; ay[r / 2].x = -2.f * y; az[r / 2].x = -2.f * z; }
+                    T[r] = (idx < ni) ? (K.rc2_hi + K.thr_margin) - fmaf(x, x, fmaf(y, y, z * z)) : -INFINITY;
                 }
-                // the pair (i, i) is not a pair
-                const int cs = cself0 + i0 + lane - t0 - st * 32;
-                if (cs >= 0 && cs < 32) word &= ~(1u << cs);
-                S.msk[st][lane] = word;
+                for (int st = 0; st < nsteps; st++) {
+                    const float4 uj = S.tile[st * 32 + lane];
+                    const float2 X = make_float2(uj.x, uj.x), Y = make_float2(uj.y, uj.y), Z = make_float2(uj.z, uj.z),
+                                 W = make_float2(uj.w, uj.w);
+#pragma unroll
+                    for (int q = 0; q < NI / 4; q++) {
+                        const float2 v0 = __ffma2_rn(ax[2 * q], X, __ffma2_rn(ay[2 * q], Y, __ffma2_rn(az[2 * q], Z, W)));
+                        const float2 v1 = __ffma2_rn(ax[2 * q + 1], X, __ffma2_rn(ay[2 * q + 1], Y, __ffma2_rn(az[2 * q + 1], Z, W)));
+                        uint4 m;
+                        m.x = __ballot_sync(FULLMASK, v0.x < T[4 * q]);
+                        m.y = __ballot_sync(FULLMASK, v0.y < T[4 * q + 1]);
+                        m.z = __ballot_sync(FULLMASK, v1.x < T[4 * q + 2]);
+                        m.w = __ballot_sync(FULLMASK, v1.y < T[4 * q + 3]);
+                        *reinterpret_cast<uint4 *>(&S.msk[st][4 * q]) = m;
+                    }
+                }
             }
             __syncwarp();
-            // ---- evaluation: lane = (atom li_, slice sl), walking its own hit bits; the next
-            // mask word is fetched one word ahead
-            int ncl = 0;
-            int st = sl, stn = sl + SL;
-            unsigned cur = (myvalid && st < nsteps) ? S.msk[st][li_] : 0u;
-            bool more = myvalid && stn < nsteps;
-            unsigned nxt = more ? S.msk[stn][li_] : 0u;
-            for (;;) {
-                if (cur == 0u && more) {
-                    cur = nxt;
-                    st = stn;
-                    stn += SL;
-                    more = stn < nsteps;
-                    nxt = more ? S.msk[stn][li_] : 0u;
-                }
-                if (!__any_sync(FULLMASK, cur != 0u || more)) break;
-                if (cur) {
-                    const int b = 31 - __clz(cur);
-                    cur &= ~(1u << b);
-                    const int c = st * 32 + b;
-                    const float4 uj = S.tile[c];
-                    const float dx = uj.x - ux, dy = uj.y - uy, dz = uj.z - uz;
-                    const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                    // p2 <= r2 < rc2_lo: FP32 term.  r2 < p2 (steep part) and the sliver around
-                    // rc^2, where FP32 could misjudge the cutoff: FP64 from exact coordinates.
-                    const bool fast = r2 >= K.p2 && r2 < K.rc2_lo;
-                    if (!fast && r2 < K.rc2_hi) {
-                        if (ncl < FC_CLOSE) S.close[ncl++][lane] = (unsigned short)c;
-                        else fc_precise(S, lpos, P, K, lme, t0, c, dfx, dfy, dfz, dpe, dw);   // queue full
-                    }
-                    const float inv = fc_rcp(r2);
-                    const float s2 = K.sig2 * inv;
-                    float s6 = s2 * s2 * s2;
-                    s6 = fast ? s6 : 0.f;
-                    float fr = inv * s6 * fmaf(K.eps48, s6, -K.eps24);
-                    if (MODE2) {
-                        const float r = sqrtf(r2);
-                        fr -= fast ? P.f_rcf * inv * r : 0.f;
-                        sR += fast ? (r - P.rcf) : 0.f;
-                    }
-                    fx = fmaf(-fr, dx, fx);
-                    fy = fmaf(-fr, dy, fy);
-                    fz = fmaf(-fr, dz, fz);
-                    sA = fmaf(s6, s6, sA);
-                    sB += s6;
-                    nin += fast;
-                }
+            // the pair (i, i) is not a pair
+            if (lane < nrow) {
+                const int cs = cself0 + i0 + lane - t0;
+                if (cs >= 0 && cs < cnt) S.msk[cs >> 5][lane] &= ~(1u << (cs & 31));
             }
-            // ---- queued close pairs in FP64 from the exact local coordinates
-            const int maxcl = __reduce_max_sync(FULLMASK, ncl);
-            for (int q = 0; q < maxcl; q++)
-                if (q < ncl) fc_precise(S, lpos, P, K, lme, t0, (int)S.close[q][lane], dfx, dfy, dfz, dpe, dw);
+            __syncwarp();
+            // ---- evaluation: lane = (atom li_, slice sl) walks the hit bits of its own mask words
+            // st = sl, sl + SL, ...; an empty word costs the lane one idle iteration
+            {
+                int ncl = 0;
+                int st = sl - SL;
+                unsigned cur = 0u;
+                bool more = myvalid;
+                for (;;) {
+                    if (cur == 0u && more) {
+                        st += SL;
+                        more = st < nsteps;
+                        if (more) {
+                            cur = S.msk[st][li_];
+                            nhit += __popc(cur);
+                        }
+                    }
+                    if (!__any_sync(FULLMASK, more)) break;
+                    if (cur) {
+                        const int b = __ffs(cur) - 1;
+                        cur &= cur - 1u;
+                        const int c = st * 32 + b;
+                        const float4 uj = S.tile[c];
+                        const float dx = uj.x - ux, dy = uj.y - uy, dz = uj.z - uz;
+                        const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                        // p2 <= r2 < rc2_lo: FP32 term.  Everything else the filter let through (the
+                        // steep part r2 < p2, the sliver around rc^2 where FP32 could misjudge the
+                        // cutoff, and false positives beyond it) is decided and evaluated in FP64.
+                        const bool fast = r2 >= K.p2 && r2 < K.rc2_lo;
+                        if (!fast) {
+                            if (ncl < FC_CLOSE) S.close[ncl++][lane] = (unsigned short)c;
+                            else fc_precise(S, lpos, P, K, lme, t0, c, dfx, dfy, dfz, dpe, dw);   // queue full
+                            nslow++;
+                        }
+                        const float inv = fc_rcp(r2);
+                        const float s2 = K.sig2 * inv;
+                        float s6 = s2 * s2 * s2;
+                        s6 = fast ? s6 : 0.f;
+                        float fr = inv * s6 * fmaf(K.eps48, s6, -K.eps24);
+                        if (MODE2) {
+                            const float r = sqrtf(r2);
+                            fr -= fast ? P.f_rcf * inv * r : 0.f;
+                            sR += fast ? (r - P.rcf) : 0.f;
+                        }
+                        fx = fmaf(-fr, dx, fx);
+                        fy = fmaf(-fr, dy, fy);
+                        fz = fmaf(-fr, dz, fz);
+                        sA = fmaf(s6, s6, sA);
+                        sB += s6;
+                    }
+                }
+                // ---- queued pairs in FP64 from the exact local coordinates
+                const int maxcl = __reduce_max_sync(FULLMASK, ncl);
+                for (int q = 0; q < maxcl; q++)
+                    if (q < ncl) fc_precise(S, lpos, P, K, lme, t0, (int)S.close[q][lane], dfx, dfy, dfz, dpe, dw);
+            }
         }
         // ---- combine the FP32 and FP64 parts, reduce over the slices, store
         // PE = 4 eps (A - B) - n ushift [+ f_rc sum(r - rc)],  W = 24 eps (2A - B) [- f_rc sum r]
+        const int nin = nhit - nslow;
         double tx = dfx + (double)fx, ty = dfy + (double)fy, tz = dfz + (double)fz;
         double pe = dpe + P.eps4 * ((double)sA - (double)sB) - (double)nin * P.ushift;
         double w = dw + P.eps24 * (2.0 * (double)sA - (double)sB);
@@ -205,13 +215,15 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
             pe += P.f_rc * (double)sR;
             w -= P.f_rc * ((double)sR + (double)nin * P.rc);
         }
-#pragma unroll
-        for (int o = G; o < 32; o <<= 1) {
-            tx += __shfl_xor_sync(FULLMASK, tx, o);
-            ty += __shfl_xor_sync(FULLMASK, ty, o);
-            tz += __shfl_xor_sync(FULLMASK, tz, o);
+        double ox = 0.0, oy = 0.0, oz = 0.0;               // totals of the other slices of my atom
+        for (int k = 1; k < SL; k++) {
+            const int src = lane + k * nrow;               // < 32 for the lanes of slice 0
+            ox += __shfl_sync(FULLMASK, tx, src);
+            oy += __shfl_sync(FULLMASK, ty, src);
+            oz += __shfl_sync(FULLMASK, tz, src);
         }
-        if (myvalid && sl == 0) frc[ibeg + myidx] = make_float4((float)tx, (float)ty, (float)tz, 0.f);
+        if (sl == 0)
+            frc[ibeg + i0 + li_] = make_float4((float)(tx + ox), (float)(ty + oy), (float)(tz + oz), 0.f);
         pe_tot += pe;
         w_tot += w;
     }

@@ -5,15 +5,6 @@
 
 #define IT 256   // threads per block for the streaming kernels
 
-// Wrap x into [0,L) after a drift of less than L (R14): a result that rounds to L becomes 0.
-__device__ __forceinline__ float wrap01(float x, float L)
-{
-    if (x >= L) x -= L;
-    else if (x < 0.0f) x += L;
-    if (x >= L || x < 0.0f) x = 0.0f;
-    return x;
-}
-
 // General wrap for md_set_state (positions may be any finite value).
 __device__ __forceinline__ float wrap_any(float x, float L)
 {
@@ -54,7 +45,10 @@ k_unpack(float *__restrict__ out, const float4 *__restrict__ src, const float4 *
     out[3 * id + 2] = a.z;
 }
 
-// a1: v += (dt/2) F;  x += dt v;  wrap.
+// a1: v += (dt/2) F;  x += dt v;  wrap.  KICKS = 2 also applies the second half-kick that the
+// previous step of the same md_step call left pending (same F, two separate FMAs, so the
+// velocities are bit-identical to the unfused sequence).
+template <int KICKS>
 __global__ void __launch_bounds__(IT)
 k_kick_drift(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4 *__restrict__ frc,
              int64_t N, float hdt, float dt, float L)
@@ -62,12 +56,15 @@ k_kick_drift(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4 *_
     int64_t i = (int64_t)blockIdx.x * IT + threadIdx.x;
     if (i >= N) return;
     float4 p = pos[i], v = vel[i], f = frc[i];
-    v.x = fmaf(hdt, f.x, v.x);
-    v.y = fmaf(hdt, f.y, v.y);
-    v.z = fmaf(hdt, f.z, v.z);
-    p.x = wrap01(fmaf(dt, v.x, p.x), L);
-    p.y = wrap01(fmaf(dt, v.y, p.y), L);
-    p.z = wrap01(fmaf(dt, v.z, p.z), L);
+#pragma unroll
+    for (int k = 0; k < KICKS; k++) {
+        v.x = fmaf(hdt, f.x, v.x);
+        v.y = fmaf(hdt, f.y, v.y);
+        v.z = fmaf(hdt, f.z, v.z);
+    }
+    p.x = wrap_drift(fmaf(dt, v.x, p.x), L);
+    p.y = wrap_drift(fmaf(dt, v.y, p.y), L);
+    p.z = wrap_drift(fmaf(dt, v.z, p.z), L);
     pos[i] = p;
     vel[i] = v;
 }
@@ -126,9 +123,12 @@ int ljmd_unpack(md_sim *s, const float4 *src, float *dout)
     return MD_OK;
 }
 
-int ljmd_kick_drift(md_sim *s)
+int ljmd_kick_drift(md_sim *s, int kicks)
 {
-    k_kick_drift<<<nblk(s->N), IT, 0, s->stream>>>(s->pos, s->vel, s->frc, s->N, s->hdtf, s->dtf, s->Lf);
+    if (kicks == 2)
+        k_kick_drift<2><<<nblk(s->N), IT, 0, s->stream>>>(s->pos, s->vel, s->frc, s->N, s->hdtf, s->dtf, s->Lf);
+    else
+        k_kick_drift<1><<<nblk(s->N), IT, 0, s->stream>>>(s->pos, s->vel, s->frc, s->N, s->hdtf, s->dtf, s->Lf);
     CKL(s);
     return MD_OK;
 }

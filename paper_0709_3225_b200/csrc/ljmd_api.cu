@@ -166,7 +166,7 @@ static void free_all(md_sim *s)
     free(s->ev_pool);
     free(s->ev_tag);
     void *ptrs[] = {s->pos, s->vel, s->frc, s->pos2, s->vel2, s->lpos, s->cell_of, s->rank, s->cell_count,
-                    s->cell_start, s->max_occ, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list,
+                    s->cell_start, s->max_occ, s->scan_ticket, s->scan_state, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list,
                     s->tile_start};
     for (void *p : ptrs) ljmd_dev_free(p, st);
 }
@@ -229,7 +229,13 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     int ncells = s->grid.n ? s->grid.ncells : 1;
     s->cell_count = (int *)ljmd_dev_alloc((size_t)ncells * sizeof(int), st);
     s->cell_start = (int *)ljmd_dev_alloc(((size_t)ncells + 1) * sizeof(int), st);
-    s->max_occ = (int *)ljmd_dev_alloc(sizeof(int), st);
+    s->max_occ = (unsigned long long *)ljmd_dev_alloc(sizeof(unsigned long long), st);
+    {
+        int nscan = ncells > s->ap_sort_bins ? ncells : s->ap_sort_bins;
+        s->scan_cap = nscan / 2048 + 2;
+    }
+    s->scan_ticket = (unsigned *)ljmd_dev_alloc(sizeof(unsigned), st);
+    s->scan_state = (unsigned long long *)ljmd_dev_alloc((size_t)s->scan_cap * sizeof(unsigned long long), st);
     s->fpart = (double *)ljmd_dev_alloc((size_t)nsplit * 3 * N * sizeof(double), st);
     s->part = (double *)ljmd_dev_alloc((size_t)3 * s->part_cap * sizeof(double), st);
     s->energies = (double *)ljmd_dev_alloc(3 * sizeof(double), st);
@@ -238,13 +244,15 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->tile_count = (int *)ljmd_dev_alloc((size_t)ntiles * sizeof(int), st);
     s->tile_start = (int *)ljmd_dev_alloc(((size_t)ntiles + 1) * sizeof(int), st);
     if (!s->tile_count || !s->tile_start || !s->pos || !s->vel || !s->frc || !s->pos2 || !s->vel2 || !s->lpos || !s->cell_of || !s->rank ||
-        !s->cell_count || !s->cell_start || !s->max_occ || !s->fpart || !s->part || !s->energies || !s->xfer) {
+        !s->cell_count || !s->cell_start || !s->max_occ || !s->scan_ticket || !s->scan_state || !s->fpart || !s->part || !s->energies || !s->xfer) {
         free_all(s);
         delete s;
         return MD_ENOMEM;
     }
     cudaError_t e = cudaMemsetAsync(s->cell_count, 0, (size_t)ncells * sizeof(int), st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(s->max_occ, 0, sizeof(int), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->max_occ, 0, sizeof(unsigned long long), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->scan_ticket, 0, sizeof(unsigned), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->scan_state, 0, (size_t)s->scan_cap * sizeof(unsigned long long), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->tile_count, 0, (size_t)ntiles * sizeof(int), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->frc, 0, f4, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -297,6 +305,7 @@ extern "C" int md_set_state(md_sim *s, const float *pos, const float *vel)
     if (r) return r;
     CK(cudaStreamSynchronize(s->stream));
     s->has_state = true;
+    s->binned = false;
     s->forces_valid = false;
     s->layout = LAYOUT_NONE;
     return MD_OK;
@@ -390,12 +399,18 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
         s->forces_algo = algo;
     }
     ljmd_tick(s, TAG_START);
+    // Inside one call the second half-kick of step k is folded into the first kernel of step
+    // k + 1 (same F, separate FMAs: bit-identical velocities); only the last step runs the
+    // half-kick + KE kernel, since intermediate kinetic energies are not observable.
     for (int64_t k = 0; k < nsteps; k++) {
-        if ((r = ljmd_kick_drift(s))) return r;
+        const int kicks = (k > 0) ? 2 : 1;
+        if ((r = (algo == MD_CELL) ? ljmd_kick_drift_bin(s, kicks) : ljmd_kick_drift(s, kicks))) return r;
         ljmd_tick(s, TAG_INTEGRATE);
         if ((r = eval_forces(s, algo))) return r;
-        if ((r = ljmd_kick_ke(s))) return r;
-        ljmd_tick(s, TAG_INTEGRATE);
+        if (k == nsteps - 1) {
+            if ((r = ljmd_kick_ke(s))) return r;
+            ljmd_tick(s, TAG_INTEGRATE);
+        }
     }
     if ((r = ljmd_reduce_energies(s))) return r;
     ljmd_tick(s, TAG_OTHER);
@@ -455,10 +470,10 @@ extern "C" int md_get_stat(md_sim *s, const char *key, double *value)
     else if (!strcmp(key, "nbr_cap")) *value = s->nbr_cap;
     else if (!strcmp(key, "n_force")) *value = (double)s->n_phase[TAG_FORCE];
     else if (!strcmp(key, "max_occupancy")) {
-        int h = 0;
-        CK(cudaMemcpyAsync(&h, s->max_occ, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+        unsigned long long h = 0;
+        CK(cudaMemcpyAsync(&h, s->max_occ, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
         CK(cudaStreamSynchronize(s->stream));
-        *value = h;
+        *value = (double)(unsigned)(h & 0xffffffffull);
     } else return MD_EINVAL;
     return MD_OK;
 }
