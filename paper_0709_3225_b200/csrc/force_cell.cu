@@ -150,59 +150,79 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
             }
             __syncwarp();
             // ---- evaluation: lane = (atom li_, slice sl) walks the hit bits of its own mask words
-            // st = sl, sl + SL, ...; an empty word costs the lane one idle iteration
+            // st = sl, sl + SL, ..., two hits per iteration (independent chains hide the LDS and
+            // MUFU latencies); an empty word costs the lane one idle iteration.
             {
                 int ncl = 0;
-                int st = sl - SL;
+                const int cend = nsteps * 32, cstride = SL * 32;
+                int cb = (sl - SL) * 32;                              // candidate index of bit 0 of `cur`
+                const unsigned *mp = &S.msk[0][0] + (sl - SL) * 16 + li_;
                 unsigned cur = 0u;
                 bool more = myvalid;
                 for (;;) {
                     if (cur == 0u && more) {
-                        st += SL;
-                        more = st < nsteps;
+                        cb += cstride;
+                        mp += SL * 16;
+                        more = cb < cend;
                         if (more) {
-                            cur = S.msk[st][li_];
+                            cur = *mp;
                             nhit += __popc(cur);
                         }
                     }
-                    if (!__any_sync(FULLMASK, more)) break;
+                    const bool done = !__any_sync(FULLMASK, more);
+                    // ---- queued pairs in FP64 from the exact local coordinates (queue nearly full, or end)
+                    if (done || ncl > FC_CLOSE - 2) {
+                        for (int q = 0; q < ncl; q++)
+                            fc_precise(S, lpos, P, K, lme, t0, (int)S.close[q][lane], dfx, dfy, dfz, dpe, dw);
+                        ncl = 0;
+                    }
+                    if (done) break;
                     if (cur) {
-                        const int b = __ffs(cur) - 1;
-                        cur &= cur - 1u;
-                        const int c = st * 32 + b;
-                        const float4 uj = S.tile[c];
-                        const float dx = uj.x - ux, dy = uj.y - uy, dz = uj.z - uz;
-                        const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                        const int b0 = 31 - __clz(cur);
+                        cur ^= 1u << b0;
+                        const bool two = cur != 0u;
+                        const int b1 = two ? 31 - __clz(cur) : b0;
+                        cur = two ? (cur ^ (1u << b1)) : 0u;
+                        const int c0 = cb + b0, c1 = cb + b1;
+                        const float4 u0 = S.tile[c0], u1 = S.tile[c1];
+                        const float dx0 = u0.x - ux, dy0 = u0.y - uy, dz0 = u0.z - uz;
+                        const float dx1 = u1.x - ux, dy1 = u1.y - uy, dz1 = u1.z - uz;
+                        const float r20 = fmaf(dx0, dx0, fmaf(dy0, dy0, dz0 * dz0));
+                        const float r21 = fmaf(dx1, dx1, fmaf(dy1, dy1, dz1 * dz1));
                         // p2 <= r2 < rc2_lo: FP32 term.  Everything else the filter let through (the
                         // steep part r2 < p2, the sliver around rc^2 where FP32 could misjudge the
                         // cutoff, and false positives beyond it) is decided and evaluated in FP64.
-                        const bool fast = r2 >= K.p2 && r2 < K.rc2_lo;
-                        if (!fast) {
-                            if (ncl < FC_CLOSE) S.close[ncl++][lane] = (unsigned short)c;
-                            else fc_precise(S, lpos, P, K, lme, t0, c, dfx, dfy, dfz, dpe, dw);   // queue full
-                            nslow++;
-                        }
-                        const float inv = fc_rcp(r2);
-                        const float s2 = K.sig2 * inv;
-                        float s6 = s2 * s2 * s2;
-                        s6 = fast ? s6 : 0.f;
-                        float fr = inv * s6 * fmaf(K.eps48, s6, -K.eps24);
+                        const bool fast0 = r20 >= K.p2 && r20 < K.rc2_lo;
+                        const bool in1 = r21 >= K.p2 && r21 < K.rc2_lo;
+                        const bool fast1 = two && in1;
+                        if (!fast0) { S.close[ncl++][lane] = (unsigned short)c0; nslow++; }
+                        if (two && !in1) { S.close[ncl++][lane] = (unsigned short)c1; nslow++; }
+                        const float inv0 = fc_rcp(r20), inv1 = fc_rcp(r21);
+                        const float s20 = K.sig2 * inv0, s21 = K.sig2 * inv1;
+                        float s60 = s20 * s20 * s20, s61 = s21 * s21 * s21;
+                        s60 = fast0 ? s60 : 0.f;
+                        s61 = fast1 ? s61 : 0.f;
+                        float fr0 = inv0 * s60 * fmaf(K.eps48, s60, -K.eps24);
+                        float fr1 = inv1 * s61 * fmaf(K.eps48, s61, -K.eps24);
                         if (MODE2) {
-                            const float r = sqrtf(r2);
-                            fr -= fast ? P.f_rcf * inv * r : 0.f;
-                            sR += fast ? (r - P.rcf) : 0.f;
+                            const float r0 = sqrtf(r20), r1 = sqrtf(r21);
+                            fr0 -= fast0 ? P.f_rcf * inv0 * r0 : 0.f;
+                            fr1 -= fast1 ? P.f_rcf * inv1 * r1 : 0.f;
+                            sR += fast0 ? (r0 - P.rcf) : 0.f;
+                            sR += fast1 ? (r1 - P.rcf) : 0.f;
                         }
-                        fx = fmaf(-fr, dx, fx);
-                        fy = fmaf(-fr, dy, fy);
-                        fz = fmaf(-fr, dz, fz);
-                        sA = fmaf(s6, s6, sA);
-                        sB += s6;
+                        fx = fmaf(-fr0, dx0, fx);
+                        fy = fmaf(-fr0, dy0, fy);
+                        fz = fmaf(-fr0, dz0, fz);
+                        sA = fmaf(s60, s60, sA);
+                        sB += s60;
+                        fx = fmaf(-fr1, dx1, fx);
+                        fy = fmaf(-fr1, dy1, fy);
+                        fz = fmaf(-fr1, dz1, fz);
+                        sA = fmaf(s61, s61, sA);
+                        sB += s61;
                     }
                 }
-                // ---- queued pairs in FP64 from the exact local coordinates
-                const int maxcl = __reduce_max_sync(FULLMASK, ncl);
-                for (int q = 0; q < maxcl; q++)
-                    if (q < ncl) fc_precise(S, lpos, P, K, lme, t0, (int)S.close[q][lane], dfx, dfy, dfz, dpe, dw);
             }
         }
         // ---- combine the FP32 and FP64 parts, reduce over the slices, store
