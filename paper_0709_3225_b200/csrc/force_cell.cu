@@ -21,19 +21,24 @@
 
 #define FC_WARPS 4
 #define FC_T (FC_WARPS * 32)
-#define FC_CAP 512                    // staged candidates per pass
+#define FC_CAP 448                    // staged candidates per pass
 #define FC_STEPS (FC_CAP / 32)
-#define FC_CLOSE 8                    // queued close pairs per lane and pass
+#define FC_CLOSE 8                    // queued FP64 pairs per lane
+#define FC_NSEG 28
+#ifndef FC_MINB
+#define FC_MINB 4
+#endif
 #define FULLMASK 0xffffffffu
 
 struct FcWarp {
-    float4 tile[FC_CAP];              // candidate in the centre cell's frame, w = |u|^2
+    float4 tile[FC_CAP];              // candidate in the centre cell's frame; w = |u|^2 with the neighbour
+                                      // cell number (0..26) in its 5 low mantissa bits
     unsigned msk[FC_STEPS][16];       // hit-mask words [32-candidate step][atom i of the pass]
     unsigned short close[FC_CLOSE][32];
-    unsigned char kk[FC_CAP];         // neighbour cell (0..26) of each staged candidate
-    float4 seg[32];                   // per neighbour cell: origin offset minus h (x, y, z) and, as int
+    float4 seg[FC_NSEG];              // per neighbour cell: origin offset minus h (x, y, z) and, as int
                                       // bits, (first slot - candidates before the cell)
-    int seg_pref[32];                 // candidates before cell k; [27] = total
+    int seg_pref[FC_NSEG];            // candidates before cell k; [27] = total
+    float rax[16], ray[16], raz[16], rT[16];   // filter rows: -2 u_i and threshold - |u_i|^2
 };
 
 struct FcConst {
@@ -54,7 +59,7 @@ __device__ __forceinline__ void fc_precise(const FcWarp &S, const float4 *__rest
                                            const FcConst &K, const float4 &lme, int t0, int c, double &fx,
                                            double &fy, double &fz, double &pe, double &w)
 {
-    const float4 sg = S.seg[S.kk[c]];
+    const float4 sg = S.seg[__float_as_int(S.tile[c].w) & 31];
     const float4 lj = lpos[__float_as_int(sg.w) + t0 + c];
     const double ex = ((double)lj.x - (double)lme.x) + ((double)sg.x + K.hd);
     const double ey = ((double)lj.y - (double)lme.y) + ((double)sg.y + K.hd);
@@ -62,28 +67,72 @@ __device__ __forceinline__ void fc_precise(const FcWarp &S, const float4 *__rest
     pair_f64(P, ex, ey, ez, fx, fy, fz, pe, w);
 }
 
-// NI: rows of the filter = atoms of the cell handled per pass (8 or 16).
-template <int NI, bool MODE2>
+// Filter: lane = candidate, rows = 4 NQ atoms (two per FFMA2), 3 FFMA + compare + ballot per
+// (atom, 32 candidates); the ballots of four rows go to shared memory as one 16-byte store
+// (every lane writes the same value).
+template <int NQ>
+__device__ __forceinline__ void fc_filter(FcWarp &S, const int nsteps, const int lane)
+{
+    float2 ax[2 * NQ], ay[2 * NQ], az[2 * NQ];
+    float4 T[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; q++) {
+        const float4 a = *reinterpret_cast<const float4 *>(&S.rax[4 * q]);
+        const float4 b = *reinterpret_cast<const float4 *>(&S.ray[4 * q]);
+        const float4 c = *reinterpret_cast<const float4 *>(&S.raz[4 * q]);
+        ax[2 * q] = make_float2(a.x, a.y); ax[2 * q + 1] = make_float2(a.z, a.w);
+        ay[2 * q] = make_float2(b.x, b.y); ay[2 * q + 1] = make_float2(b.z, b.w);
+        az[2 * q] = make_float2(c.x, c.y); az[2 * q + 1] = make_float2(c.z, c.w);
+        T[q] = *reinterpret_cast<const float4 *>(&S.rT[4 * q]);
+    }
+    for (int st = 0; st < nsteps; st++) {
+        const float4 uj = S.tile[st * 32 + lane];
+        const float2 X = make_float2(uj.x, uj.x), Y = make_float2(uj.y, uj.y), Z = make_float2(uj.z, uj.z),
+                     W = make_float2(uj.w, uj.w);
+#pragma unroll
+        for (int q = 0; q < NQ; q++) {
+            const float2 v0 = __ffma2_rn(ax[2 * q], X, __ffma2_rn(ay[2 * q], Y, __ffma2_rn(az[2 * q], Z, W)));
+            const float2 v1 = __ffma2_rn(ax[2 * q + 1], X, __ffma2_rn(ay[2 * q + 1], Y, __ffma2_rn(az[2 * q + 1], Z, W)));
+            uint4 m;
+            m.x = __ballot_sync(FULLMASK, v0.x < T[q].x);
+            m.y = __ballot_sync(FULLMASK, v0.y < T[q].y);
+            m.z = __ballot_sync(FULLMASK, v1.x < T[q].z);
+            m.w = __ballot_sync(FULLMASK, v1.y < T[q].w);
+            *reinterpret_cast<uint4 *>(&S.msk[st][4 * q]) = m;
+        }
+    }
+}
+
+template <bool MODE2>
 __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lpos, const int ibeg, const int ni,
                                         const int total, const int mycnt, const PairParams &P, const FcConst &K,
                                         float4 *__restrict__ frc, double &pe_tot, double &w_tot)
 {
     const int lane = threadIdx.x & 31;
     const int cself0 = S.seg_pref[13];                  // candidate index of the cell's own atom 0
-    const int mypref = S.seg_pref[lane];
+    const int mypref = (lane < FC_NSEG) ? S.seg_pref[lane] : total;
     int staged_t0 = -1;
 
-    for (int i0 = 0; i0 < ni; i0 += NI) {
+    for (int i0 = 0; i0 < ni; i0 += 16) {
         // evaluation mapping of this pass: nrow atoms, SL slices of the mask words per atom
-        const int nrow = min(NI, ni - i0);
+        const int nrow = min(16, ni - i0);
         const int SL = 32 / nrow;
         const int sl = lane / nrow, li_ = lane - sl * nrow;
         const bool myvalid = sl < SL;
         const float4 lme = lpos[ibeg + i0 + li_];
         const float ux = lme.x - K.h, uy = lme.y - K.h, uz = lme.z - K.h;
-        float fx = 0.f, fy = 0.f, fz = 0.f, sA = 0.f, sB = 0.f, sR = 0.f;   // sums of s^12, s^6, (r - rc)
-        int nhit = 0, nslow = 0;
-        double dfx = 0.0, dfy = 0.0, dfz = 0.0, dpe = 0.0, dw = 0.0;
+        double tx = 0.0, ty = 0.0, tz = 0.0, pe = 0.0, w = 0.0;      // this lane's totals over the passes
+        // rows of the filter for this pass (lane r < 16 prepares row r)
+        __syncwarp();
+        if (lane < 16) {
+            const int idx = i0 + lane;
+            const float4 l = lpos[ibeg + min(idx, ni - 1)];
+            const float x = l.x - K.h, y = l.y - K.h, z = l.z - K.h;
+            S.rax[lane] = -2.f * x;
+            S.ray[lane] = -2.f * y;
+            S.raz[lane] = -2.f * z;
+            S.rT[lane] = (idx < ni) ? (K.rc2_hi + K.thr_margin) - fmaf(x, x, fmaf(y, y, z * z)) : -INFINITY;
+        }
 
         for (int t0 = 0; t0 < total; t0 += FC_CAP) {
             const int cnt = min(FC_CAP, total - t0);
@@ -94,54 +143,44 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
                 __syncwarp();
                 {   // lane k < 27 labels the candidates of its cell
                     const int lo = max(mypref, t0) - t0, hi = min(mypref + mycnt, t0 + cnt) - t0;
-                    for (int c = lo; c < hi; c++) S.kk[c] = (unsigned char)lane;
+                    for (int c = lo; c < hi; c++) S.tile[c].w = __int_as_float(lane);
                 }
                 __syncwarp();
-                for (int c = lane; c < nsteps * 32; c += 32) {
-                    float4 u = make_float4(0.f, 0.f, 0.f, INFINITY);
-                    if (c < cnt) {
-                        const float4 sg = S.seg[S.kk[c]];
-                        const float4 l = lpos[__float_as_int(sg.w) + t0 + c];
-                        u.x = l.x + sg.x;
-                        u.y = l.y + sg.y;
-                        u.z = l.z + sg.z;
-                        u.w = fmaf(u.x, u.x, fmaf(u.y, u.y, u.z * u.z));
+                // four candidates per lane and batch: all loads are issued before the first store
+                for (int c0 = lane; c0 < nsteps * 32; c0 += 128) {
+                    float4 l[4], sg[4];
+                    int kq[4];
+#pragma unroll
+                    for (int u = 0; u < 4; u++) {
+                        const int c = c0 + 32 * u;
+                        kq[u] = (c < cnt) ? __float_as_int(S.tile[c].w) : 0;
                     }
-                    S.tile[c] = u;
+#pragma unroll
+                    for (int u = 0; u < 4; u++) sg[u] = S.seg[kq[u]];
+#pragma unroll
+                    for (int u = 0; u < 4; u++) {
+                        const int c = c0 + 32 * u;
+                        l[u] = lpos[__float_as_int(sg[u].w) + t0 + min(c, cnt - 1)];
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; u++) {
+                        const int c = c0 + 32 * u;
+                        float4 v;
+                        v.x = l[u].x + sg[u].x;
+                        v.y = l[u].y + sg[u].y;
+                        v.z = l[u].z + sg[u].z;
+                        v.w = fmaf(v.x, v.x, fmaf(v.y, v.y, v.z * v.z));
+                        v.w = __int_as_float((__float_as_int(v.w) & ~31) | kq[u]);
+                        if (c >= cnt) v = make_float4(0.f, 0.f, 0.f, INFINITY);
+                        if (c < nsteps * 32) S.tile[c] = v;
+                    }
                 }
             }
             __syncwarp();
-            // ---- filter: lane = candidate, rows = atoms (two per FFMA2); the ballots of four rows
-            // go to shared memory as one 16-byte store (every lane writes the same value)
-            {
-                float2 ax[NI / 2], ay[NI / 2], az[NI / 2];
-                float T[NI];
-#pragma unroll
-                for (int r = 0; r < NI; r++) {
-                    const int idx = i0 + r;
-                    const float4 l = lpos[ibeg + min(idx, ni - 1)];
-                    const float x = l.x - K.h, y = l.y - K.h, z = l.z - K.h;
-                    if (r & 1) { ax[r / 2].y = -2.f * x; ay[r / 2].y = -2.f * y; az[r / 2].y = -2.f * z; }
-                    else { ax[r / 2].x = -2.f * x; ay[r / 2].x = -2.f * y; az[r / 2].x = -2.f * z; }
-                    T[r] = (idx < ni) ? (K.rc2_hi + K.thr_margin) - fmaf(x, x, fmaf(y, y, z * z)) : -INFINITY;
-                }
-                for (int st = 0; st < nsteps; st++) {
-                    const float4 uj = S.tile[st * 32 + lane];
-                    const float2 X = make_float2(uj.x, uj.x), Y = make_float2(uj.y, uj.y), Z = make_float2(uj.z, uj.z),
-                                 W = make_float2(uj.w, uj.w);
-#pragma unroll
-                    for (int q = 0; q < NI / 4; q++) {
-                        const float2 v0 = __ffma2_rn(ax[2 * q], X, __ffma2_rn(ay[2 * q], Y, __ffma2_rn(az[2 * q], Z, W)));
-                        const float2 v1 = __ffma2_rn(ax[2 * q + 1], X, __ffma2_rn(ay[2 * q + 1], Y, __ffma2_rn(az[2 * q + 1], Z, W)));
-                        uint4 m;
-                        m.x = __ballot_sync(FULLMASK, v0.x < T[4 * q]);
-                        m.y = __ballot_sync(FULLMASK, v0.y < T[4 * q + 1]);
-                        m.z = __ballot_sync(FULLMASK, v1.x < T[4 * q + 2]);
-                        m.w = __ballot_sync(FULLMASK, v1.y < T[4 * q + 3]);
-                        *reinterpret_cast<uint4 *>(&S.msk[st][4 * q]) = m;
-                    }
-                }
-            }
+            if (nrow <= 4) fc_filter<1>(S, nsteps, lane);
+            else if (nrow <= 8) fc_filter<2>(S, nsteps, lane);
+            else if (nrow <= 12) fc_filter<3>(S, nsteps, lane);
+            else fc_filter<4>(S, nsteps, lane);
             __syncwarp();
             // the pair (i, i) is not a pair
             if (lane < nrow) {
@@ -152,89 +191,119 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
             // ---- evaluation: lane = (atom li_, slice sl) walks the hit bits of its own mask words
             // st = sl, sl + SL, ..., two hits per iteration (independent chains hide the LDS and
             // MUFU latencies); an empty word costs the lane one idle iteration.
+            float fx = 0.f, fy = 0.f, fz = 0.f, sA = 0.f, sB = 0.f, sR = 0.f;   // sums of s^12, s^6, (r - rc)
+            int nhit = 0, ncl = 0;
             {
-                int ncl = 0;
-                const int cend = nsteps * 32, cstride = SL * 32;
-                int cb = (sl - SL) * 32;                              // candidate index of bit 0 of `cur`
-                const unsigned *mp = &S.msk[0][0] + (sl - SL) * 16 + li_;
-                unsigned cur = 0u;
-                bool more = myvalid;
-                for (;;) {
-                    if (cur == 0u && more) {
+                // Branch-free walk: `cur` holds the unprocessed bits of the current word (candidates
+                // cb .. cb + 31), `nxt` the prefetched next word of the slice, `rem` the words after it.
+                const int cstride = SL * 32;
+                const int nwords = (myvalid && sl < nsteps) ? (nsteps - 1 - sl) / SL + 1 : 0;   // st = sl, sl + SL, ...
+                int cb = nwords ? sl * 32 : 0;
+                const unsigned *mp = &S.msk[0][0] + (nwords ? sl * 16 : 0) + li_;
+                int rem = nwords - 1;                                   // words after the current one
+                unsigned cur = (rem >= 0) ? *mp : 0u;
+                unsigned nxt = (rem >= 1) ? mp[SL * 16] : 0u;
+                mp += SL * 16;
+                nhit = __popc(cur);
+                while (__any_sync(FULLMASK, (cur != 0u) | (rem > 0))) {
+                    const bool v0 = cur != 0u;
+                    const int b0 = v0 ? 31 - __clz(cur) : 0;
+                    cur &= ~(1u << b0);
+                    const bool v1 = cur != 0u;
+                    const int b1 = v1 ? 31 - __clz(cur) : b0;
+                    cur &= ~(1u << b1);
+                    const int c0 = cb + b0, c1 = cb + b1;
+                    const float4 u0 = S.tile[c0], u1 = S.tile[c1];
+                    // refill for the next iteration while the pair terms are in flight
+                    const bool need = (cur == 0u) & (rem > 0);
+                    if (need) {
+                        cur = nxt;
                         cb += cstride;
+                        rem--;
                         mp += SL * 16;
-                        more = cb < cend;
-                        if (more) {
-                            cur = *mp;
-                            nhit += __popc(cur);
-                        }
+                        nhit += __popc(nxt);
+                        nxt = (rem > 0) ? *mp : 0u;
                     }
-                    const bool done = !__any_sync(FULLMASK, more);
-                    // ---- queued pairs in FP64 from the exact local coordinates (queue nearly full, or end)
-                    if (done || ncl > FC_CLOSE - 2) {
-                        for (int q = 0; q < ncl; q++)
-                            fc_precise(S, lpos, P, K, lme, t0, (int)S.close[q][lane], dfx, dfy, dfz, dpe, dw);
-                        ncl = 0;
+                    const float dx0 = u0.x - ux, dy0 = u0.y - uy, dz0 = u0.z - uz;
+                    const float dx1 = u1.x - ux, dy1 = u1.y - uy, dz1 = u1.z - uz;
+                    // an idle slot (no bit left) computes on r2 = 1 and contributes nothing
+                    const float r20 = v0 ? fmaf(dx0, dx0, fmaf(dy0, dy0, dz0 * dz0)) : 1.f;
+                    const float r21 = v1 ? fmaf(dx1, dx1, fmaf(dy1, dy1, dz1 * dz1)) : 1.f;
+                    // p2 <= r2 < rc2_lo: FP32 term.  Everything else the filter let through (the
+                    // steep part r2 < p2, the sliver around rc^2 where FP32 could misjudge the
+                    // cutoff, and false positives beyond it) is decided and evaluated in FP64.
+                    const bool in0 = r20 >= K.p2 && r20 < K.rc2_lo;
+                    const bool in1 = r21 >= K.p2 && r21 < K.rc2_lo;
+                    const bool fast0 = v0 && in0, fast1 = v1 && in1;
+                    if (v0 && !in0) S.close[min(ncl++, FC_CLOSE - 1)][lane] = (unsigned short)c0;
+                    if (v1 && !in1) S.close[min(ncl++, FC_CLOSE - 1)][lane] = (unsigned short)c1;
+                    const float inv0 = fc_rcp(r20), inv1 = fc_rcp(r21);
+                    const float s20 = K.sig2 * inv0, s21 = K.sig2 * inv1;
+                    float s60 = s20 * s20 * s20, s61 = s21 * s21 * s21;
+                    s60 = fast0 ? s60 : 0.f;
+                    s61 = fast1 ? s61 : 0.f;
+                    float fr0 = inv0 * s60 * fmaf(K.eps48, s60, -K.eps24);
+                    float fr1 = inv1 * s61 * fmaf(K.eps48, s61, -K.eps24);
+                    if (MODE2) {
+                        const float r0 = sqrtf(r20), r1 = sqrtf(r21);
+                        fr0 -= fast0 ? P.f_rcf * inv0 * r0 : 0.f;
+                        fr1 -= fast1 ? P.f_rcf * inv1 * r1 : 0.f;
+                        sR += fast0 ? (r0 - P.rcf) : 0.f;
+                        sR += fast1 ? (r1 - P.rcf) : 0.f;
                     }
-                    if (done) break;
-                    if (cur) {
-                        const int b0 = 31 - __clz(cur);
-                        cur ^= 1u << b0;
-                        const bool two = cur != 0u;
-                        const int b1 = two ? 31 - __clz(cur) : b0;
-                        cur = two ? (cur ^ (1u << b1)) : 0u;
-                        const int c0 = cb + b0, c1 = cb + b1;
-                        const float4 u0 = S.tile[c0], u1 = S.tile[c1];
-                        const float dx0 = u0.x - ux, dy0 = u0.y - uy, dz0 = u0.z - uz;
-                        const float dx1 = u1.x - ux, dy1 = u1.y - uy, dz1 = u1.z - uz;
-                        const float r20 = fmaf(dx0, dx0, fmaf(dy0, dy0, dz0 * dz0));
-                        const float r21 = fmaf(dx1, dx1, fmaf(dy1, dy1, dz1 * dz1));
-                        // p2 <= r2 < rc2_lo: FP32 term.  Everything else the filter let through (the
-                        // steep part r2 < p2, the sliver around rc^2 where FP32 could misjudge the
-                        // cutoff, and false positives beyond it) is decided and evaluated in FP64.
-                        const bool fast0 = r20 >= K.p2 && r20 < K.rc2_lo;
-                        const bool in1 = r21 >= K.p2 && r21 < K.rc2_lo;
-                        const bool fast1 = two && in1;
-                        if (!fast0) { S.close[ncl++][lane] = (unsigned short)c0; nslow++; }
-                        if (two && !in1) { S.close[ncl++][lane] = (unsigned short)c1; nslow++; }
-                        const float inv0 = fc_rcp(r20), inv1 = fc_rcp(r21);
-                        const float s20 = K.sig2 * inv0, s21 = K.sig2 * inv1;
-                        float s60 = s20 * s20 * s20, s61 = s21 * s21 * s21;
-                        s60 = fast0 ? s60 : 0.f;
-                        s61 = fast1 ? s61 : 0.f;
-                        float fr0 = inv0 * s60 * fmaf(K.eps48, s60, -K.eps24);
-                        float fr1 = inv1 * s61 * fmaf(K.eps48, s61, -K.eps24);
-                        if (MODE2) {
-                            const float r0 = sqrtf(r20), r1 = sqrtf(r21);
-                            fr0 -= fast0 ? P.f_rcf * inv0 * r0 : 0.f;
-                            fr1 -= fast1 ? P.f_rcf * inv1 * r1 : 0.f;
-                            sR += fast0 ? (r0 - P.rcf) : 0.f;
-                            sR += fast1 ? (r1 - P.rcf) : 0.f;
+                    fx = fmaf(-fr0, dx0, fx);
+                    fy = fmaf(-fr0, dy0, fy);
+                    fz = fmaf(-fr0, dz0, fz);
+                    sA = fmaf(s60, s60, sA);
+                    sB += s60;
+                    fx = fmaf(-fr1, dx1, fx);
+                    fy = fmaf(-fr1, dy1, fy);
+                    fz = fmaf(-fr1, dz1, fz);
+                    sA = fmaf(s61, s61, sA);
+                    sB += s61;
+                }
+            }
+            // ---- FP64 part of this pass.  Queued pairs from the exact local coordinates; a lane
+            // whose queue overflowed (more than FC_CLOSE slow pairs: very rare) instead rescans its
+            // mask words and takes every pair outside the FP32 window.
+            double dfx = 0.0, dfy = 0.0, dfz = 0.0, dpe = 0.0, dw = 0.0;
+            {
+                const bool ovf = ncl > FC_CLOSE;
+                const int nq = ovf ? 0 : ncl;
+                const int maxq = __reduce_max_sync(FULLMASK, nq);
+                for (int q = 0; q < maxq; q++)
+                    if (q < nq) fc_precise(S, lpos, P, K, lme, t0, (int)S.close[q][lane], dfx, dfy, dfz, dpe, dw);
+                if (__any_sync(FULLMASK, ovf)) {
+                    if (ovf) {
+                        for (int st = sl; st < nsteps; st += SL) {
+                            unsigned m = S.msk[st][li_];
+                            while (m) {
+                                const int b = __ffs(m) - 1;
+                                m &= m - 1u;
+                                const int c = st * 32 + b;
+                                const float4 uj = S.tile[c];
+                                const float dx = uj.x - ux, dy = uj.y - uy, dz = uj.z - uz;
+                                const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                                if (!(r2 >= K.p2 && r2 < K.rc2_lo))
+                                    fc_precise(S, lpos, P, K, lme, t0, c, dfx, dfy, dfz, dpe, dw);
+                            }
                         }
-                        fx = fmaf(-fr0, dx0, fx);
-                        fy = fmaf(-fr0, dy0, fy);
-                        fz = fmaf(-fr0, dz0, fz);
-                        sA = fmaf(s60, s60, sA);
-                        sB += s60;
-                        fx = fmaf(-fr1, dx1, fx);
-                        fy = fmaf(-fr1, dy1, fy);
-                        fz = fmaf(-fr1, dz1, fz);
-                        sA = fmaf(s61, s61, sA);
-                        sB += s61;
                     }
                 }
             }
+            // PE = 4 eps (A - B) - n ushift [+ f_rc sum(r - rc)],  W = 24 eps (2A - B) [- f_rc sum r]
+            const int nin = nhit - ncl;
+            tx += dfx + (double)fx;
+            ty += dfy + (double)fy;
+            tz += dfz + (double)fz;
+            pe += dpe + P.eps4 * ((double)sA - (double)sB) - (double)nin * P.ushift;
+            w += dw + P.eps24 * (2.0 * (double)sA - (double)sB);
+            if (MODE2) {
+                pe += P.f_rc * (double)sR;
+                w -= P.f_rc * ((double)sR + (double)nin * P.rc);
+            }
         }
-        // ---- combine the FP32 and FP64 parts, reduce over the slices, store
-        // PE = 4 eps (A - B) - n ushift [+ f_rc sum(r - rc)],  W = 24 eps (2A - B) [- f_rc sum r]
-        const int nin = nhit - nslow;
-        double tx = dfx + (double)fx, ty = dfy + (double)fy, tz = dfz + (double)fz;
-        double pe = dpe + P.eps4 * ((double)sA - (double)sB) - (double)nin * P.ushift;
-        double w = dw + P.eps24 * (2.0 * (double)sA - (double)sB);
-        if (MODE2) {
-            pe += P.f_rc * (double)sR;
-            w -= P.f_rc * ((double)sR + (double)nin * P.rc);
-        }
+        // ---- reduce over the slices, store
         double ox = 0.0, oy = 0.0, oz = 0.0;               // totals of the other slices of my atom
         for (int k = 1; k < SL; k++) {
             const int src = lane + k * nrow;               // < 32 for the lanes of slice 0
@@ -250,7 +319,7 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
 }
 
 template <bool MODE2>
-__global__ void __launch_bounds__(FC_T, 4)
+__global__ void __launch_bounds__(FC_T, FC_MINB)
 k_force_cell_warp(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, int ncells, Grid g,
                   PairParams P, FcConst K, float4 *__restrict__ frc, double *__restrict__ part_pe,
                   double *__restrict__ part_w)
@@ -291,11 +360,12 @@ k_force_cell_warp(const float4 *__restrict__ lpos, const int *__restrict__ cell_
             }
             const int total = __shfl_sync(FULLMASK, incl, 31);
             const int pref = incl - cnt;                 // lanes >= 27: total
-            S.seg_pref[lane] = pref;
-            S.seg[lane] = make_float4(ox - K.h, oy - K.h, oz - K.h, __int_as_float(start - pref));
+            if (lane < FC_NSEG) {
+                S.seg_pref[lane] = pref;
+                S.seg[lane] = make_float4(ox - K.h, oy - K.h, oz - K.h, __int_as_float(start - pref));
+            }
             __syncwarp();
-            if (ni <= 8) fc_cell<8, MODE2>(S, lpos, ibeg, ni, total, cnt, P, K, frc, pe, w);
-            else fc_cell<16, MODE2>(S, lpos, ibeg, ni, total, cnt, P, K, frc, pe, w);
+            fc_cell<MODE2>(S, lpos, ibeg, ni, total, cnt, P, K, frc, pe, w);
         }
     }
     pe = block_sum(pe, red);
@@ -321,7 +391,8 @@ int ljmd_forces_cell(md_sim *s)
     K.h = 0.5f * s->grid.side;
     K.hd = (double)K.h;
     const double reach = 1.5 * (double)s->grid.last;
-    K.thr_margin = (float)(1e-5 * 3.0 * reach * reach + 1e-6 * P.rc2);
+    // FP32 rounding of the expanded form plus the 5 mantissa bits of |u|^2 that carry the cell number
+    K.thr_margin = (float)(1.5e-5 * 3.0 * reach * reach + 1e-6 * P.rc2);
     K.sig2 = P.sig2f;
     K.eps24 = P.eps24f;
     K.eps48 = 2.0f * P.eps24f;
