@@ -31,7 +31,7 @@
 #define FULLMASK 0xffffffffu
 
 struct FcWarp {
-    float4 tile[FC_CAP];              // candidate in the centre cell's frame; w = |u|^2 with the neighbour
+    float4 tile[FC_CAP + 1];          // [FC_CAP] = dummy far-away entry for idle slots; candidate in the centre cell's frame; w = |u|^2 with the neighbour
                                       // cell number (0..26) in its 5 low mantissa bits
     unsigned msk[FC_STEPS][16];       // hit-mask words [32-candidate step][atom i of the pass]
     unsigned short close[FC_CLOSE][32];
@@ -52,6 +52,13 @@ __device__ __forceinline__ float fc_rcp(float x)      // 1/x, x normal and posit
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     const float e = fmaf(-x, y, 1.f);
     return fmaf(y, e, y);
+}
+
+__device__ __forceinline__ int fc_top_bit(unsigned x)      // index of the highest set bit (x != 0): one FLO
+{
+    int b;
+    asm("bfind.u32 %0, %1;" : "=r"(b) : "r"(x));
+    return b;
 }
 
 // FP64 pair term of my atom (exact local coordinates lme) with staged candidate c of pass t0
@@ -206,13 +213,15 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
                 mp += SL * 16;
                 nhit = __popc(cur);
                 while (__any_sync(FULLMASK, (cur != 0u) | (rem > 0))) {
+                    // an idle slot (no bit left) reads the dummy entry behind the tile: far away, finite
                     const bool v0 = cur != 0u;
-                    const int b0 = v0 ? 31 - __clz(cur) : 0;
-                    cur &= ~(1u << b0);
+                    const int b0 = fc_top_bit(cur);
+                    const int c0 = v0 ? cb + b0 : FC_CAP;
+                    cur = v0 ? (cur ^ (1u << b0)) : 0u;
                     const bool v1 = cur != 0u;
-                    const int b1 = v1 ? 31 - __clz(cur) : b0;
-                    cur &= ~(1u << b1);
-                    const int c0 = cb + b0, c1 = cb + b1;
+                    const int b1 = fc_top_bit(cur);
+                    const int c1 = v1 ? cb + b1 : FC_CAP;
+                    cur = v1 ? (cur ^ (1u << b1)) : 0u;
                     const float4 u0 = S.tile[c0], u1 = S.tile[c1];
                     // refill for the next iteration while the pair terms are in flight
                     const bool need = (cur == 0u) & (rem > 0);
@@ -226,15 +235,14 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
                     }
                     const float dx0 = u0.x - ux, dy0 = u0.y - uy, dz0 = u0.z - uz;
                     const float dx1 = u1.x - ux, dy1 = u1.y - uy, dz1 = u1.z - uz;
-                    // an idle slot (no bit left) computes on r2 = 1 and contributes nothing
-                    const float r20 = v0 ? fmaf(dx0, dx0, fmaf(dy0, dy0, dz0 * dz0)) : 1.f;
-                    const float r21 = v1 ? fmaf(dx1, dx1, fmaf(dy1, dy1, dz1 * dz1)) : 1.f;
+                    const float r20 = fmaf(dx0, dx0, fmaf(dy0, dy0, dz0 * dz0));
+                    const float r21 = fmaf(dx1, dx1, fmaf(dy1, dy1, dz1 * dz1));
                     // p2 <= r2 < rc2_lo: FP32 term.  Everything else the filter let through (the
                     // steep part r2 < p2, the sliver around rc^2 where FP32 could misjudge the
                     // cutoff, and false positives beyond it) is decided and evaluated in FP64.
                     const bool in0 = r20 >= K.p2 && r20 < K.rc2_lo;
                     const bool in1 = r21 >= K.p2 && r21 < K.rc2_lo;
-                    const bool fast0 = v0 && in0, fast1 = v1 && in1;
+                    const bool fast0 = in0, fast1 = in1;             // the dummy entry is never in range
                     if (v0 && !in0) S.close[min(ncl++, FC_CLOSE - 1)][lane] = (unsigned short)c0;
                     if (v1 && !in1) S.close[min(ncl++, FC_CLOSE - 1)][lane] = (unsigned short)c1;
                     const float inv0 = fc_rcp(r20), inv1 = fc_rcp(r21);
@@ -360,6 +368,7 @@ k_force_cell_warp(const float4 *__restrict__ lpos, const int *__restrict__ cell_
             }
             const int total = __shfl_sync(FULLMASK, incl, 31);
             const int pref = incl - cnt;                 // lanes >= 27: total
+            if (lane == 31) S.tile[FC_CAP] = make_float4(1.0e4f, 1.0e4f, 1.0e4f, INFINITY);
             if (lane < FC_NSEG) {
                 S.seg_pref[lane] = pref;
                 S.seg[lane] = make_float4(ox - K.h, oy - K.h, oz - K.h, __int_as_float(start - pref));
