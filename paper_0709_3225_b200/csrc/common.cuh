@@ -93,6 +93,7 @@ struct md_sim {
     int forces_algo;
     bool use_graph;
     int sort_every;
+    int cell_group;               // cells per row group of the cell-force kernel; 0 = automatic
     int64_t launches, steps_done;
     // CUDA graph cache for one step
     cudaGraphExec_t graph_exec[2];

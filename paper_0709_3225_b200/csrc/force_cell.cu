@@ -24,7 +24,8 @@
 #define FC_CAP 448                    // staged candidates per pass
 #define FC_STEPS (FC_CAP / 32)
 #define FC_CLOSE 8                    // queued FP64 pairs per lane
-#define FC_NSEG 28
+#define FC_KZ_MAX 4                   // cells per row group
+#define FC_NSEG (9 * (FC_KZ_MAX + 2) + 2)
 #ifndef FC_MINB
 #define FC_MINB 4
 #endif
@@ -32,19 +33,35 @@
 
 struct FcWarp {
     float4 tile[FC_CAP + 1];          // [FC_CAP] = dummy far-away entry for idle slots; candidate in the centre cell's frame; w = |u|^2 with the neighbour
-                                      // cell number (0..26) in its 5 low mantissa bits
+                                      // segment number (0..53) in its 6 low mantissa bits
     unsigned msk[FC_STEPS][16];       // hit-mask words [32-candidate step][atom i of the pass]
     unsigned short close[FC_CLOSE][32];
-    float4 seg[FC_NSEG];              // per neighbour cell: origin offset minus h (x, y, z) and, as int
+    float4 seg[FC_NSEG];              // per segment (neighbour cell): origin offset minus h (x, y, z) and, as int
                                       // bits, (first slot - candidates before the cell)
-    int seg_pref[FC_NSEG];            // candidates before cell k; [27] = total
+    int seg_pref[FC_NSEG];            // candidates before segment k; [nseg ..] = total
     float rax[16], ray[16], raz[16], rT[16];   // filter rows: -2 u_i and threshold - |u_i|^2
 };
 
 struct FcConst {
     float rc2_lo, rc2_hi, p2, thr_margin, sig2, eps24, eps48, h;   // [rc2_lo, rc2_hi): decided in FP64
     double hd;
+    int kz, nzu;                      // cells per row group, row groups per z-column
 };
+
+struct FcGroup {                      // one warp's row group
+    int ibeg, ni, total, kk, cfirst;  // first slot, atoms, candidates, cells, first cell
+    float hz, side;                   // z centre of the group in the frame of its first cell
+    double hzd;
+    int pref0, cnt0, pref1, cnt1;     // this lane's two segments (lane, lane + 32)
+};
+
+// z offset of row atom `slot` inside the group: (its cell - first cell) * side, exact
+__device__ __forceinline__ float fc_row_zoff(const int *__restrict__ cell_start, const FcGroup &G, int slot)
+{
+    int q = 0;
+    for (int k = 1; k < G.kk; k++) q += (slot >= cell_start[G.cfirst + k]) ? 1 : 0;
+    return (float)q * G.side;
+}
 
 __device__ __forceinline__ float fc_rcp(float x)      // 1/x, x normal and positive: MUFU + one Newton step
 {
@@ -63,14 +80,14 @@ __device__ __forceinline__ int fc_top_bit(unsigned x)      // index of the highe
 
 // FP64 pair term of my atom (exact local coordinates lme) with staged candidate c of pass t0
 __device__ __forceinline__ void fc_precise(const FcWarp &S, const float4 *__restrict__ lpos, const PairParams &P,
-                                           const FcConst &K, const float4 &lme, int t0, int c, double &fx,
-                                           double &fy, double &fz, double &pe, double &w)
+                                           const FcConst &K, const float4 &lme, const double zme, int t0, int c,
+                                           double &fx, double &fy, double &fz, double &pe, double &w)
 {
-    const float4 sg = S.seg[__float_as_int(S.tile[c].w) & 31];
+    const float4 sg = S.seg[__float_as_int(S.tile[c].w) & 63];
     const float4 lj = lpos[__float_as_int(sg.w) + t0 + c];
     const double ex = ((double)lj.x - (double)lme.x) + ((double)sg.x + K.hd);
     const double ey = ((double)lj.y - (double)lme.y) + ((double)sg.y + K.hd);
-    const double ez = ((double)lj.z - (double)lme.z) + ((double)sg.z + K.hd);
+    const double ez = ((double)lj.z - (double)lme.z) + ((double)sg.z + zme);     // zme = hz - my z offset
     pair_f64(P, ex, ey, ez, fx, fy, fz, pe, w);
 }
 
@@ -111,13 +128,13 @@ __device__ __forceinline__ void fc_filter(FcWarp &S, const int nsteps, const int
 }
 
 template <bool MODE2>
-__device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lpos, const int ibeg, const int ni,
-                                        const int total, const int mycnt, const PairParams &P, const FcConst &K,
-                                        float4 *__restrict__ frc, double &pe_tot, double &w_tot)
+__device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lpos,
+                                        const int *__restrict__ cell_start, const FcGroup &G, const PairParams &P,
+                                        const FcConst &K, float4 *__restrict__ frc, double &pe_tot, double &w_tot)
 {
     const int lane = threadIdx.x & 31;
-    const int cself0 = S.seg_pref[13];                  // candidate index of the cell's own atom 0
-    const int mypref = (lane < FC_NSEG) ? S.seg_pref[lane] : total;
+    const int ibeg = G.ibeg, ni = G.ni, total = G.total;
+    const int cself0 = S.seg_pref[4 * (G.kk + 2) + 1];  // candidate index of the group's own atom 0
     int staged_t0 = -1;
 
     for (int i0 = 0; i0 < ni; i0 += 16) {
@@ -127,14 +144,17 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
         const int sl = lane / nrow, li_ = lane - sl * nrow;
         const bool myvalid = sl < SL;
         const float4 lme = lpos[ibeg + i0 + li_];
-        const float ux = lme.x - K.h, uy = lme.y - K.h, uz = lme.z - K.h;
+        const float zoff_me = fc_row_zoff(cell_start, G, ibeg + i0 + li_);
+        const float ux = lme.x - K.h, uy = lme.y - K.h, uz = (lme.z + zoff_me) - G.hz;
+        const double zme = G.hzd - (double)zoff_me;
         double tx = 0.0, ty = 0.0, tz = 0.0, pe = 0.0, w = 0.0;      // this lane's totals over the passes
         // rows of the filter for this pass (lane r < 16 prepares row r)
         __syncwarp();
         if (lane < 16) {
             const int idx = i0 + lane;
-            const float4 l = lpos[ibeg + min(idx, ni - 1)];
-            const float x = l.x - K.h, y = l.y - K.h, z = l.z - K.h;
+            const int slot = ibeg + min(idx, ni - 1);
+            const float4 l = lpos[slot];
+            const float x = l.x - K.h, y = l.y - K.h, z = (l.z + fc_row_zoff(cell_start, G, slot)) - G.hz;
             S.rax[lane] = -2.f * x;
             S.ray[lane] = -2.f * y;
             S.raz[lane] = -2.f * z;
@@ -148,9 +168,13 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
                 // ---- stage the candidates t0 .. t0 + cnt of the concatenated neighbour cells
                 staged_t0 = t0;
                 __syncwarp();
-                {   // lane k < 27 labels the candidates of its cell
-                    const int lo = max(mypref, t0) - t0, hi = min(mypref + mycnt, t0 + cnt) - t0;
+                {   // every lane labels the candidates of its two segments
+                    int lo = max(G.pref0, t0) - t0, hi = min(G.pref0 + G.cnt0, t0 + cnt) - t0;
                     for (int c = lo; c < hi; c++) S.tile[c].w = __int_as_float(lane);
+                    if (G.kk > 1) {
+                        lo = max(G.pref1, t0) - t0, hi = min(G.pref1 + G.cnt1, t0 + cnt) - t0;
+                        for (int c = lo; c < hi; c++) S.tile[c].w = __int_as_float(lane + 32);
+                    }
                 }
                 __syncwarp();
                 // four candidates per lane and batch: all loads are issued before the first store
@@ -177,7 +201,7 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
                         v.y = l[u].y + sg[u].y;
                         v.z = l[u].z + sg[u].z;
                         v.w = fmaf(v.x, v.x, fmaf(v.y, v.y, v.z * v.z));
-                        v.w = __int_as_float((__float_as_int(v.w) & ~31) | kq[u]);
+                        v.w = __int_as_float((__float_as_int(v.w) & ~63) | kq[u]);
                         if (c >= cnt) v = make_float4(0.f, 0.f, 0.f, INFINITY);
                         if (c < nsteps * 32) S.tile[c] = v;
                     }
@@ -280,7 +304,7 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
                 const int nq = ovf ? 0 : ncl;
                 const int maxq = __reduce_max_sync(FULLMASK, nq);
                 for (int q = 0; q < maxq; q++)
-                    if (q < nq) fc_precise(S, lpos, P, K, lme, t0, (int)S.close[q][lane], dfx, dfy, dfz, dpe, dw);
+                    if (q < nq) fc_precise(S, lpos, P, K, lme, zme, t0, (int)S.close[q][lane], dfx, dfy, dfz, dpe, dw);
                 if (__any_sync(FULLMASK, ovf)) {
                     if (ovf) {
                         for (int st = sl; st < nsteps; st += SL) {
@@ -293,7 +317,7 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
                                 const float dx = uj.x - ux, dy = uj.y - uy, dz = uj.z - uz;
                                 const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
                                 if (!(r2 >= K.p2 && r2 < K.rc2_lo))
-                                    fc_precise(S, lpos, P, K, lme, t0, c, dfx, dfy, dfz, dpe, dw);
+                                    fc_precise(S, lpos, P, K, lme, zme, t0, c, dfx, dfy, dfz, dpe, dw);
                             }
                         }
                     }
@@ -326,70 +350,114 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
     }
 }
 
+// One warp per "row group": kk <= K.kz consecutive cells of one z-column (contiguous slots, since
+// z runs fastest in the cell numbering).  kz = 1 is the paper's block-per-cell;
+// kz > 1 packs sparsely filled cells into one set of filter rows.  The candidates are the
+// 9 columns x (kk + 2) cells around the group, i.e. the union of its cells' 27 neighbours.
+// grid = (ceil(nzu / FC_WARPS), n, n): blockIdx.z = cx, blockIdx.y = cy.
 template <bool MODE2>
 __global__ void __launch_bounds__(FC_T, FC_MINB)
-k_force_cell_warp(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, int ncells, Grid g,
+k_force_cell_warp(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, Grid g,
                   PairParams P, FcConst K, float4 *__restrict__ frc, double *__restrict__ part_pe,
                   double *__restrict__ part_w)
 {
     __shared__ FcWarp sm[FC_WARPS];
-    __shared__ double red[32];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int c = blockIdx.x * FC_WARPS + wid;
+    const int zu = blockIdx.x * FC_WARPS + wid;
+    const int n = g.n, cx = blockIdx.z, cy = blockIdx.y;
     double pe = 0.0, w = 0.0;
-    if (c < ncells) {
-        const int ibeg = cell_start[c], ni = cell_start[c + 1] - ibeg;
+    if (zu < K.nzu) {
+        const int z0 = zu * K.kz, kk = min(K.kz, n - z0);
+        const int cfirst = (cx * n + cy) * n + z0;
+        const int ibeg = cell_start[cfirst], ni = cell_start[cfirst + kk] - ibeg;
         if (ni > 0) {
             FcWarp &S = sm[wid];
-            // the 27 neighbour cells, one per lane: slot range and origin offset
-            const int n = g.n;
-            const int cz = c % n, cy = (c / n) % n, cx = c / (n * n);
-            int cnt = 0, start = 0;
-            float ox = 0.f, oy = 0.f, oz = 0.f;
-            if (lane < 27) {
-                const int ax = lane / 9 - 1, ay = (lane / 3) % 3 - 1, az = lane % 3 - 1;
-                int nx = cx + ax, ny = cy + ay, nz = cz + az;
-                nx += (nx < 0) ? n : 0; nx -= (nx >= n) ? n : 0;
-                ny += (ny < 0) ? n : 0; ny -= (ny >= n) ? n : 0;
-                nz += (nz < 0) ? n : 0; nz -= (nz >= n) ? n : 0;
-                // distance between the two cell origins: exact
-                ox = (ax == 0) ? 0.f : (ax > 0 ? ((cx == n - 1) ? g.last : g.side) : -((nx == n - 1) ? g.last : g.side));
-                oy = (ay == 0) ? 0.f : (ay > 0 ? ((cy == n - 1) ? g.last : g.side) : -((ny == n - 1) ? g.last : g.side));
-                oz = (az == 0) ? 0.f : (az > 0 ? ((cz == n - 1) ? g.last : g.side) : -((nz == n - 1) ? g.last : g.side));
-                const int nb = (nx * n + ny) * n + nz;
-                start = cell_start[nb];
-                cnt = cell_start[nb + 1] - start;
-            }
-            int incl = cnt;
+            const int nz2 = kk + 2, nseg = 9 * nz2;
+            const float hz = 0.5f * (float)kk * g.side;              // centre of the group in its frame
+            int cnt[2], start[2], incl[2];
+            float4 off[2];
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int y = __shfl_up_sync(FULLMASK, incl, o);
-                if (lane >= o) incl += y;
+            for (int h = 0; h < 2; h++) {
+                const int sgi = lane + 32 * h;                        // segment = (column, dz)
+                cnt[h] = 0; start[h] = 0;
+                off[h] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if ((h == 0 || nseg > 32) && sgi < nseg) {
+                    const int col = sgi / nz2, dz = sgi - col * nz2 - 1;     // dz = -1 .. kk
+                    const int ax = col / 3 - 1, ay = col - (col / 3) * 3 - 1;
+                    int nx = cx + ax, ny = cy + ay, nz = z0 + dz;
+                    nx += (nx < 0) ? n : 0; nx -= (nx >= n) ? n : 0;
+                    ny += (ny < 0) ? n : 0; ny -= (ny >= n) ? n : 0;
+                    nz += (nz < 0) ? n : 0; nz -= (nz >= n) ? n : 0;
+                    // distance between the cell origins: exact
+                    off[h].x = (ax == 0) ? 0.f : (ax > 0 ? ((cx == n - 1) ? g.last : g.side) : -((nx == n - 1) ? g.last : g.side));
+                    off[h].y = (ay == 0) ? 0.f : (ay > 0 ? ((cy == n - 1) ? g.last : g.side) : -((ny == n - 1) ? g.last : g.side));
+                    float oz;
+                    if (dz < 0) oz = -((nz == n - 1) ? g.last : g.side);
+                    else oz = (float)dz * g.side + ((dz > 0 && z0 + dz - 1 == n - 1) ? (g.last - g.side) : 0.f);
+                    off[h].z = oz;
+                    const int nb = (nx * n + ny) * n + nz;
+                    start[h] = cell_start[nb];
+                    cnt[h] = cell_start[nb + 1] - start[h];
+                }
             }
-            const int total = __shfl_sync(FULLMASK, incl, 31);
-            const int pref = incl - cnt;                 // lanes >= 27: total
+            int carry = 0;
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                int v = cnt[h];
+                if (h == 0 || nseg > 32) {                           // warp-uniform
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int y = __shfl_up_sync(FULLMASK, v, o);
+                        if (lane >= o) v += y;
+                    }
+                }
+                incl[h] = v + carry;
+                carry += (h == 0 || nseg > 32) ? __shfl_sync(FULLMASK, v, 31) : 0;
+            }
+            const int total = carry;
             if (lane == 31) S.tile[FC_CAP] = make_float4(1.0e4f, 1.0e4f, 1.0e4f, INFINITY);
-            if (lane < FC_NSEG) {
-                S.seg_pref[lane] = pref;
-                S.seg[lane] = make_float4(ox - K.h, oy - K.h, oz - K.h, __int_as_float(start - pref));
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                const int sgi = lane + 32 * h;
+                if (sgi < FC_NSEG) {
+                    const int pref = incl[h] - cnt[h];                // segments >= nseg: total
+                    S.seg_pref[sgi] = pref;
+                    S.seg[sgi] = make_float4(off[h].x - K.h, off[h].y - K.h, off[h].z - hz,
+                                             __int_as_float(start[h] - pref));
+                }
             }
             __syncwarp();
-            fc_cell<MODE2>(S, lpos, ibeg, ni, total, cnt, P, K, frc, pe, w);
+            FcGroup G;
+            G.ibeg = ibeg; G.ni = ni; G.total = total; G.kk = kk; G.cfirst = cfirst;
+            G.hz = hz; G.hzd = (double)hz; G.side = g.side;
+            G.pref0 = incl[0] - cnt[0]; G.cnt0 = cnt[0]; G.pref1 = incl[1] - cnt[1]; G.cnt1 = cnt[1];
+            fc_cell<MODE2>(S, lpos, cell_start, G, P, K, frc, pe, w);
         }
     }
-    pe = block_sum(pe, red);
-    w = block_sum(w, red);
-    if (threadIdx.x == 0) {
-        part_pe[blockIdx.x] = 0.5 * pe;              // every pair is visited from both ends
-        part_w[blockIdx.x] = 0.5 * w;
+    pe = warp_sum(pe);
+    w = warp_sum(w);
+    if (lane == 0) {
+        const int u = (cx * n + cy) * (gridDim.x * FC_WARPS) + zu;
+        part_pe[u] = 0.5 * pe;                       // every pair is visited from both ends
+        part_w[u] = 0.5 * w;
     }
 }
 
 int ljmd_forces_cell(md_sim *s)
 {
-    const int ncells = s->grid.ncells;
-    const int nb = (ncells + FC_WARPS - 1) / FC_WARPS;
-    if (nb > s->part_cap) return MD_ENOMEM;
+    const Grid &g = s->grid;
+    // cells per row group: fill the 16 filter rows on average (option "cell_group" overrides)
+    int kz = s->cell_group;
+    if (kz <= 0) {
+        const double occ = (double)s->N / (double)g.ncells;
+        kz = (int)(18.0 / (occ > 0.5 ? occ : 0.5) + 0.5);
+    }
+    if (kz > FC_KZ_MAX) kz = FC_KZ_MAX;
+    if (kz < 1 || g.n < 8) kz = 1;                  // dz * side must stay exact in FP32 (L >= 16)
+    const int nzu = (g.n + kz - 1) / kz;
+    const dim3 grid((nzu + FC_WARPS - 1) / FC_WARPS, g.n, g.n);
+    const int64_t nunits = (int64_t)grid.x * FC_WARPS * g.n * g.n;
+    if (nunits > s->part_cap) return MD_ENOMEM;
     double *ppe = s->part + (size_t)s->part_cap;
     double *pw = s->part + 2 * (size_t)s->part_cap;
     const PairParams &P = s->pp;
@@ -397,20 +465,23 @@ int ljmd_forces_cell(md_sim *s)
     K.rc2_lo = (float)(P.rc2 * (1.0 - 4e-6));
     K.rc2_hi = (float)(P.rc2 * (1.0 + 4e-6));
     K.p2 = (float)fmin(P.precise_r2, 3.0e38);
-    K.h = 0.5f * s->grid.side;
+    K.h = 0.5f * g.side;
     K.hd = (double)K.h;
-    const double reach = 1.5 * (double)s->grid.last;
-    // FP32 rounding of the expanded form plus the 5 mantissa bits of |u|^2 that carry the cell number
-    K.thr_margin = (float)(1.5e-5 * 3.0 * reach * reach + 1e-6 * P.rc2);
+    K.kz = kz;
+    K.nzu = nzu;
+    // farthest staged candidate from the frame centre, per dimension
+    const double reach_xy = 1.5 * (double)g.last, reach_z = (0.5 * kz + 1.0) * (double)g.last;
+    // FP32 rounding of the expanded form plus the 6 mantissa bits of |u|^2 that carry the segment number
+    K.thr_margin = (float)(2.0e-5 * (2.0 * reach_xy * reach_xy + reach_z * reach_z) + 1e-6 * P.rc2);
     K.sig2 = P.sig2f;
     K.eps24 = P.eps24f;
     K.eps48 = 2.0f * P.eps24f;
     if (P.mode == 2)
-        k_force_cell_warp<true><<<nb, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, ncells, s->grid, P, K, s->frc, ppe, pw);
+        k_force_cell_warp<true><<<grid, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, g, P, K, s->frc, ppe, pw);
     else
-        k_force_cell_warp<false><<<nb, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, ncells, s->grid, P, K, s->frc, ppe, pw);
+        k_force_cell_warp<false><<<grid, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, g, P, K, s->frc, ppe, pw);
     CKL(s);
     ljmd_tick(s, TAG_FORCE);
-    s->n_pe = nb;
+    s->n_pe = (int)nunits;
     return MD_OK;
 }

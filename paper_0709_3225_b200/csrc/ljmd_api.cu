@@ -214,7 +214,10 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     if ((int)((N + 7) / 8) > cap_ap) cap_ap = (int)((N + 7) / 8);       // k_allpairs_eval: 8 atoms per block
     int cap_it = (int)((N + 255) / 256);
     s->part_cap = (cap_ap > cap_it ? cap_ap : cap_it) + 64;
-    if (s->grid.n && s->grid.ncells / 4 + 64 > s->part_cap) s->part_cap = s->grid.ncells / 4 + 64;   // one partial per 4 cells
+    if (s->grid.n) {                                                   // one partial per row group (warp)
+        int64_t nu = (int64_t)s->grid.n * s->grid.n * (s->grid.n + 3) + 64;
+        if (nu > s->part_cap) s->part_cap = (int)nu;
+    }
 
     cudaStream_t st = s->stream;
     size_t f4 = (size_t)N * sizeof(float4);
@@ -441,6 +444,9 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
         if (R != 1 && R != 2 && R != 4 && R != 8) return MD_EINVAL;
         ljmd_ap_set_R(s, R);
         s->layout = LAYOUT_NONE;
+    } else if (!strcmp(key, "cell_group")) {
+        if (value < 0 || value > 4) return MD_EINVAL;
+        s->cell_group = (int)value;
     } else if (!strcmp(key, "sort_every")) {
         if (value < 1) return MD_EINVAL;
         s->sort_every = (int)value;
