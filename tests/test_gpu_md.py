@@ -82,6 +82,20 @@ def test_forces_cell_tiling_and_precision_modes(b, n, rho, amp, precise_r2):
     assert w == pytest.approx(wo, rel=rel, abs=1e-9)
 
 
+@pytest.mark.parametrize("n,rho,amp", [(16, 0.3, 0.15), (14, 0.1, 0.3), (13, 0.8, 0.1)])
+@pytest.mark.parametrize("kz", [1, 2, 3, 4])
+def test_forces_cell_row_groups(b, n, rho, amp, kz):
+    """Row groups of kz cells per warp (option "cell_group"): same forces for every kz, including
+    groups that touch the periodic seam in z and the ragged last group of a column."""
+    pos, L = wl.perturbed_fcc(n, rho, amp, seed=900 + n)
+    vel = np.zeros_like(pos)
+    F, (ke, pe, w) = gpu_forces(b, pos, vel, L, b.MD_CELL, 1, opts=(("cell_group", kz),))
+    Fo, peo, wo = oracle.forces(pos.astype(np.float64), L, algo=1)
+    nviol, worst = force_check(F, Fo)
+    assert nviol == 0, (nviol, worst)
+    assert pe == pytest.approx(peo, rel=1e-6) and w == pytest.approx(wo, rel=1e-6)
+
+
 @pytest.mark.parametrize("n,rho,amp", [(7, 0.9, 0.08), (10, 0.8, 0.1), (12, 0.8, 0.1), (16, 0.5, 0.12)])
 @pytest.mark.parametrize("R", [1, 2, 4, 8])
 def test_allpairs_sorted_kernel_matches_general_and_oracle(b, n, rho, amp, R):
