@@ -339,11 +339,28 @@ k_allpairs_filter(const float4 *__restrict__ pos, int N, float rc, float rc2, fl
 #pragma unroll 4
                 for (int k = 0; k < 32; k += 2) {
                     const float4 a = tc[k], b = tc[k + 1];
+                    if constexpr (R >= 2) {
+                        // two atoms per FFMA2 (same IEEE fma per half as the scalar rescan below)
+                        const float2 aX = make_float2(a.x, a.x), aY = make_float2(a.y, a.y), aZ = make_float2(a.z, a.z),
+                                     aW = make_float2(a.w, a.w);
+                        const float2 bX = make_float2(b.x, b.x), bY = make_float2(b.y, b.y), bZ = make_float2(b.z, b.z),
+                                     bW = make_float2(b.w, b.w);
 #pragma unroll
-                    for (int r = 0; r < R; r++) {
-                        float v1 = fmaf(ax[r], a.x, fmaf(ay[r], a.y, fmaf(az[r], a.z, a.w)));
-                        float v2 = fmaf(ax[r], b.x, fmaf(ay[r], b.y, fmaf(az[r], b.z, b.w)));
-                        m[r] = fminf(m[r], fminf(v1, v2));
+                        for (int q = 0; q < R / 2; q++) {
+                            const float2 x2 = make_float2(ax[2 * q], ax[2 * q + 1]), y2 = make_float2(ay[2 * q], ay[2 * q + 1]),
+                                         z2 = make_float2(az[2 * q], az[2 * q + 1]);
+                            const float2 v1 = __ffma2_rn(x2, aX, __ffma2_rn(y2, aY, __ffma2_rn(z2, aZ, aW)));
+                            const float2 v2 = __ffma2_rn(x2, bX, __ffma2_rn(y2, bY, __ffma2_rn(z2, bZ, bW)));
+                            m[2 * q] = fminf(m[2 * q], fminf(v1.x, v2.x));
+                            m[2 * q + 1] = fminf(m[2 * q + 1], fminf(v1.y, v2.y));
+                        }
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < R; r++) {
+                            float v1 = fmaf(ax[r], a.x, fmaf(ay[r], a.y, fmaf(az[r], a.z, a.w)));
+                            float v2 = fmaf(ax[r], b.x, fmaf(ay[r], b.y, fmaf(az[r], b.z, b.w)));
+                            m[r] = fminf(m[r], fminf(v1, v2));
+                        }
                     }
                 }
                 bool hit = false;
