@@ -41,6 +41,19 @@ def measured_peaks():
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
 
 
+def ncu_traffic(workload):
+    """DRAM bytes per launch of the workload's dominant kernel, from the committed ncu --set full
+    summary (profiles/r01_traffic_v3.txt; it is measured under ncu, so it cannot be taken live)."""
+    p = os.path.join(ROOT, "profiles", "r01_traffic_v3.txt")
+    if not os.path.exists(p):
+        return None
+    for ln in open(p):
+        f = ln.split()
+        if len(f) == 3 and f[0] == workload:
+            return float(f[2])
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -266,6 +279,7 @@ def run_ours(args):
         with b.Sim(N, sysd["L"]) as tmp:
             ncell = int(tmp.stat("ncell"))
         roof = cell_roofline(N, cfg["rho"], wl.RC, ncell, r["t_force_kernel_ms"], peaks, n_sms)
+    roof["traffic"] = ncu_traffic(name)
     roof["kernel_ms"] = r["t_force_kernel_ms"]
     roof["kernel_share_of_step"] = r["phases_ms"]["force"] / max(1e-12, sum(r["phases_ms"].values()))
 
