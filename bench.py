@@ -104,6 +104,20 @@ def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
 
 
+def max_over_ranks(vals, dist, device):
+    """Element-wise MAX of a list of timings over all ranks (the only collective of the bench:
+    replicas share no data).  Works on any backend (nccl on GPUs, gloo in tests)."""
+    import torch
+    t = torch.tensor(list(vals), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.cpu()]
+
+
+def whole_job_value(n_units_per_rank, world, ms_max):
+    """Aggregate throughput of `world` independent replicas: units all ranks processed / slowest rank's time."""
+    return world * n_units_per_rank / (ms_max * 1e-3)
+
+
 # ----------------------------------------------------------------------------- our arm
 def flush_l2(torch, buf):
     buf.add_(1)           # read + write 256 MB: larger than the 126 MB L2
@@ -268,11 +282,9 @@ def run_ours(args):
     ms = r["flushed_ms"]
     e2e = time_md_e2e(b, torch, sysd, algo, min(steps, 50))
     if world > 1:
-        t = torch.tensor([ms, r["steady_ms"], e2e["ms_per_step"]], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, r["steady_ms"], e2e["ms_per_step"] = [float(x) for x in t.cpu()]
+        ms, r["steady_ms"], e2e["ms_per_step"] = max_over_ranks([ms, r["steady_ms"], e2e["ms_per_step"]], dist, "cuda")
     N = sysd["N"]
-    value = world * N / (ms * 1e-3)
+    value = whole_job_value(N, world, ms)
     if algo == 0:
         roof = allpairs_roofline(N, cfg["rho"], wl.RC, r["t_force_kernel_ms"], peaks, n_sms)
     else:
