@@ -110,7 +110,12 @@ typedef void (*md_free_fn)(void *ptr, void *cuda_stream);
 int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
 
 /* Tuning and introspection.  md_set_option keys:
- *   "graph"          1 (default) replay each step from a CUDA graph, 0 launch directly
+ *   "graph"          1 (default): inside one md_step call the interior steps (all but the first and
+ *                    the last) are replayed from a CUDA graph that holds one unit of steps (2 on the
+ *                    cell path, 2 * sort_every on the sorted all-pairs path: the number of steps
+ *                    after which the buffer roles repeat); 0 = launch every kernel directly
+ *   "cell_group"     cells of one z-column handled by one warp of the cell-force kernel (1..4);
+ *                    0 (default) = chosen from the mean occupancy
  *   "time_kernels"   1 = record CUDA events around every phase of md_step (disables the graph);
  *                    read back with md_get_stat "t_force_ms", "t_build_ms", "t_integrate_ms",
  *                    "t_other_ms", "n_force"; setting it resets the accumulators
@@ -121,7 +126,8 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
  *   "ap_R"           atoms per thread (1, 2, 4, 8) of the sorted all-pairs kernel, overriding the
  *                    choice made from N and L; blocks too wide for the box test per-pair images
  * md_get_stat keys: "ncell" (cells per dimension), "max_occupancy", "kernel_launches"
- * (kernels launched by this handle so far), "steps_done", "side" (cell side). */
+ * (kernels launched by this handle so far, graph nodes included), "graph_replays", "steps_done",
+ * "side" (cell side). */
 int md_set_option(md_sim *s, const char *key, double value);
 int md_get_stat(md_sim *s, const char *key, double *value);
 

@@ -61,7 +61,9 @@ k_kick_drift_bin(float4 *__restrict__ pos, float4 *__restrict__ vel, const float
 // counters for the next build.  Single pass over any number of cells: blocks take tiles of
 // SC_TILE cells in ticket order and chain their prefixes through `state` with a decoupled
 // look-back (one 64-bit word per tile: value | kind << 32 | epoch << 34, so words of earlier
-// launches read as "empty" and nothing has to be cleared between launches).
+// launches read as "empty" and nothing has to be cleared between launches).  The ticket base and
+// the epoch live in device memory and are advanced by the last block to finish, so the launch has
+// no per-call host arguments and can be replayed from a CUDA graph.
 #define SC_T 256
 #define SC_ITEMS 8
 #define SC_TILE (SC_T * SC_ITEMS)
@@ -75,16 +77,22 @@ __device__ __forceinline__ unsigned long long sc_word(unsigned long long epoch, 
 
 __global__ void __launch_bounds__(SC_T)
 k_scan_cells(int *__restrict__ cell_count, int *__restrict__ cell_start, int ncells,
-             unsigned long long *__restrict__ max_occ,
-             unsigned *__restrict__ ticket, unsigned ticket_base, volatile unsigned long long *__restrict__ state,
-             unsigned long long epoch)
+             unsigned long long *__restrict__ max_occ, ScanCtl *__restrict__ ctl,
+             volatile unsigned long long *__restrict__ state)
 {
     __shared__ int wsum[SC_T / 32];
     __shared__ int s_tile, s_prefix;
+    __shared__ unsigned s_base;
+    __shared__ unsigned long long s_epoch;
     const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
-    if (t == 0) s_tile = (int)(atomicAdd(ticket, 1u) - ticket_base);
+    if (t == 0) {
+        s_base = *(volatile unsigned *)&ctl->base;             // stable while any block of this launch runs
+        s_epoch = *(volatile unsigned long long *)&ctl->epoch;
+        s_tile = (int)(atomicAdd(&ctl->ticket, 1u) - s_base);
+    }
     __syncthreads();
     const int tile = s_tile;
+    const unsigned long long epoch = s_epoch;
     const int base = tile * SC_TILE + t * SC_ITEMS;      // SC_ITEMS consecutive cells per thread
     int v[SC_ITEMS];
     int sum = 0, mx = 0;
@@ -166,6 +174,18 @@ k_scan_cells(int *__restrict__ cell_count, int *__restrict__ cell_start, int nce
             if (base + k < ncells) { cell_start[base + k] = o[k]; cell_count[base + k] = 0; }
         if (base < ncells) cell_start[ncells] = run;      // the thread holding the last cell
     }
+    // the last block to finish opens the next launch: new ticket base, next epoch
+    __syncthreads();
+    if (t == 0) {
+        __threadfence();
+        if (atomicAdd(&ctl->done, 1u) == gridDim.x - 1) {
+            ctl->done = 0u;
+            ctl->base = s_base + gridDim.x;
+            const unsigned long long e1 = (epoch + 1ull) & 0x3fffffffull;
+            ctl->epoch = e1 ? e1 : 1ull;                               // 0 marks never-written words
+            __threadfence();
+        }
+    }
 }
 
 // Scatter into cell order: state (global coordinates) and cell-local coordinates.
@@ -194,10 +214,7 @@ int ljmd_scan_counts(md_sim *s, int *count, int *start, int n)
 {
     const int nb = (n + SC_TILE - 1) / SC_TILE;
     if (nb > s->scan_cap) return MD_ENOMEM;
-    s->scan_epoch++;
-    k_scan_cells<<<nb, SC_T, 0, s->stream>>>(count, start, n, s->max_occ, s->scan_ticket, s->scan_ticket_base,
-                                             s->scan_state, (unsigned long long)(s->scan_epoch & 0x3fffffff));
-    s->scan_ticket_base += (unsigned)nb;
+    k_scan_cells<<<nb, SC_T, 0, s->stream>>>(count, start, n, s->max_occ, s->scan_ctl, s->scan_state);
     CKL(s);
     return MD_OK;
 }

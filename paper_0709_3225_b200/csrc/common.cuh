@@ -42,6 +42,25 @@ struct Grid {
     float L;
 };
 
+// One cached graph: valid for this force path and exactly this host-side state at the unit's start
+#define MD_NGRAPH 4
+struct GraphEntry {
+    cudaGraphExec_t exec;
+    int algo, unit, since_sort, layout, stamp;
+    void *pos, *vel;
+    int64_t launches;             // kernels per replay
+    cudaStream_t stream;
+};
+
+// Control block of k_scan_cells (device memory; cells.cu)
+struct ScanCtl {
+    unsigned ticket;              // monotonic block ticket counter
+    unsigned base;                // ticket of tile 0 of the current launch
+    unsigned done;                // blocks of the current launch that have finished
+    unsigned pad;
+    unsigned long long epoch;     // launch number (30 bits), tags the look-back words and max_occ
+};
+
 enum { TAG_START = -1, TAG_INTEGRATE = 0, TAG_BUILD = 1, TAG_FORCE = 2, TAG_OTHER = 3, TAG_FORCE2 = 4, TAG_COUNT = 5 };
 
 struct md_sim {
@@ -63,12 +82,10 @@ struct md_sim {
     int *cell_count;              // [ncells]
     int *cell_start;              // [ncells + 1]
     unsigned long long *max_occ;  // [1] epoch << 32 | max cell occupancy of the last scan
-    // multi-block scan: ticket counter, per-tile look-back words, launch epoch
-    unsigned *scan_ticket;
-    unsigned scan_ticket_base;
+    // multi-block scan: device-side control block and per-tile look-back words
+    ScanCtl *scan_ctl;
     unsigned long long *scan_state;
     int scan_cap;
-    unsigned long long scan_epoch;
     // all-pairs partial forces: [nsplit][3][N] doubles
     double *fpart;
     int ap_nsplit;                // j splits of the general kernel
@@ -95,9 +112,12 @@ struct md_sim {
     int sort_every;
     int cell_group;               // cells per row group of the cell-force kernel; 0 = automatic
     int64_t launches, steps_done;
-    // CUDA graph cache for one step
-    cudaGraphExec_t graph_exec[2];
-    bool graph_ok[2];
+    // CUDA graphs of one "unit" of interior steps (ljmd_api.cu): the unit is the number of steps after
+    // which the host-side state (buffer roles, re-sort phase) repeats, so the graph can be replayed
+    GraphEntry graphs[MD_NGRAPH];
+    int graph_clock;              // LRU stamp
+    cudaStream_t cap_stream;      // capture/replay stream when the caller's stream is the legacy default
+    int64_t graph_replays;
     // optional per-phase timing with CUDA events on s->stream ("time_kernels" option)
     bool time_kernels;
     cudaEvent_t *ev_pool;

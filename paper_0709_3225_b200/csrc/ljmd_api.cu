@@ -157,16 +157,25 @@ int ljmd_collect_ticks(md_sim *s)
 }
 
 // ---- create / destroy -----------------------------------------------------------------
+static void drop_graphs(md_sim *s)
+{
+    for (int k = 0; k < MD_NGRAPH; k++) {
+        if (s->graphs[k].exec) cudaGraphExecDestroy(s->graphs[k].exec);
+        memset(&s->graphs[k], 0, sizeof(GraphEntry));
+    }
+}
+
 static void free_all(md_sim *s)
 {
     cudaStream_t st = s->stream;
-    for (int k = 0; k < 2; k++)
-        if (s->graph_exec[k]) cudaGraphExecDestroy(s->graph_exec[k]);
+    for (int k = 0; k < MD_NGRAPH; k++)
+        if (s->graphs[k].exec) cudaGraphExecDestroy(s->graphs[k].exec);
+    if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     for (int k = 0; k < s->ev_cap; k++) cudaEventDestroy(s->ev_pool[k]);
     free(s->ev_pool);
     free(s->ev_tag);
     void *ptrs[] = {s->pos, s->vel, s->frc, s->pos2, s->vel2, s->lpos, s->cell_of, s->rank, s->cell_count,
-                    s->cell_start, s->max_occ, s->scan_ticket, s->scan_state, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list,
+                    s->cell_start, s->max_occ, s->scan_ctl, s->scan_state, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list,
                     s->tile_start};
     for (void *p : ptrs) ljmd_dev_free(p, st);
 }
@@ -237,7 +246,7 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
         int nscan = ncells > s->ap_sort_bins ? ncells : s->ap_sort_bins;
         s->scan_cap = nscan / 2048 + 2;
     }
-    s->scan_ticket = (unsigned *)ljmd_dev_alloc(sizeof(unsigned), st);
+    s->scan_ctl = (ScanCtl *)ljmd_dev_alloc(sizeof(ScanCtl), st);
     s->scan_state = (unsigned long long *)ljmd_dev_alloc((size_t)s->scan_cap * sizeof(unsigned long long), st);
     s->fpart = (double *)ljmd_dev_alloc((size_t)nsplit * 3 * N * sizeof(double), st);
     s->part = (double *)ljmd_dev_alloc((size_t)3 * s->part_cap * sizeof(double), st);
@@ -247,14 +256,20 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->tile_count = (int *)ljmd_dev_alloc((size_t)ntiles * sizeof(int), st);
     s->tile_start = (int *)ljmd_dev_alloc(((size_t)ntiles + 1) * sizeof(int), st);
     if (!s->tile_count || !s->tile_start || !s->pos || !s->vel || !s->frc || !s->pos2 || !s->vel2 || !s->lpos || !s->cell_of || !s->rank ||
-        !s->cell_count || !s->cell_start || !s->max_occ || !s->scan_ticket || !s->scan_state || !s->fpart || !s->part || !s->energies || !s->xfer) {
+        !s->cell_count || !s->cell_start || !s->max_occ || !s->scan_ctl || !s->scan_state || !s->fpart || !s->part || !s->energies || !s->xfer) {
         free_all(s);
         delete s;
         return MD_ENOMEM;
     }
     cudaError_t e = cudaMemsetAsync(s->cell_count, 0, (size_t)ncells * sizeof(int), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->max_occ, 0, sizeof(unsigned long long), st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(s->scan_ticket, 0, sizeof(unsigned), st);
+    if (e == cudaSuccess) {
+        ScanCtl c0;
+        memset(&c0, 0, sizeof(c0));
+        c0.epoch = 1;                                               // 0 marks never-written look-back words
+        e = cudaMemcpyAsync(s->scan_ctl, &c0, sizeof(c0), cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);         // c0 is on the stack
+    }
     if (e == cudaSuccess) e = cudaMemsetAsync(s->scan_state, 0, (size_t)s->scan_cap * sizeof(unsigned long long), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->tile_count, 0, (size_t)ntiles * sizeof(int), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->frc, 0, f4, st);
@@ -283,7 +298,7 @@ extern "C" int md_set_stream(md_sim *s, void *stream)
     if (!s) return MD_EINVAL;
     CK(cudaStreamSynchronize(s->stream));
     s->stream = (cudaStream_t)stream;
-    for (int k = 0; k < 2; k++) s->graph_ok[k] = false;
+    drop_graphs(s);
     return MD_OK;
 }
 
@@ -374,6 +389,109 @@ static int eval_forces(md_sim *s, int algo)
     return MD_OK;
 }
 
+// One velocity-Verlet step: [pending half-kick +] half-kick + drift [+ histogram], forces,
+// and on the last step of a call the closing half-kick + KE.
+static int one_step(md_sim *s, int algo, int kicks, bool last)
+{
+    int r;
+    if ((r = (algo == MD_CELL) ? ljmd_kick_drift_bin(s, kicks) : ljmd_kick_drift(s, kicks))) return r;
+    ljmd_tick(s, TAG_INTEGRATE);
+    if ((r = eval_forces(s, algo))) return r;
+    if (last) {
+        if ((r = ljmd_kick_ke(s))) return r;
+        ljmd_tick(s, TAG_INTEGRATE);
+    }
+    return MD_OK;
+}
+
+// Steps after which the host-side state repeats: the cell build swaps the pos/vel buffer roles
+// every step; the all-pairs path re-sorts (and swaps) every sort_every steps.
+static int graph_unit(const md_sim *s, int algo)
+{
+    if (algo == MD_CELL) return 2;
+    if (s->ap_tiled && !s->ap_force_general) return 2 * s->sort_every;
+    return 1;
+}
+
+// Replay up to `nunits` units of interior steps from a cached (or newly captured) graph.
+// *done = steps advanced (0 if graphs turned out to be unusable: the caller launches directly).
+static int replay_interior(md_sim *s, int algo, int unit, int64_t nunits, int64_t *done)
+{
+    *done = 0;
+    cudaStream_t user = s->stream, run = user;
+    if (user == nullptr || user == cudaStreamLegacy) {
+        // the legacy default stream cannot be captured: use a blocking stream, which the legacy
+        // stream orders itself against in both directions
+        if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamDefault) != cudaSuccess) {
+            cudaGetLastError();
+            s->use_graph = false;
+            return MD_OK;
+        }
+        run = s->cap_stream;
+    }
+    GraphEntry *g = nullptr;
+    for (int i = 0; i < MD_NGRAPH; i++) {
+        GraphEntry &e = s->graphs[i];
+        if (e.exec && e.algo == algo && e.unit == unit && e.pos == (void *)s->pos && e.vel == (void *)s->vel &&
+            e.since_sort == s->ap_since_sort && e.layout == s->layout && e.stream == run)
+            g = &e;
+    }
+    if (!g) {
+        // capture one unit by running the ordinary host code on the capturing stream; the
+        // host-side state it leaves equals the state it found (that is what defines the unit)
+        int victim = 0;
+        for (int i = 1; i < MD_NGRAPH; i++)
+            if (s->graphs[i].stamp < s->graphs[victim].stamp) victim = i;
+        GraphEntry e;
+        memset(&e, 0, sizeof(e));
+        e.algo = algo; e.unit = unit; e.pos = s->pos; e.vel = s->vel; e.since_sort = s->ap_since_sort;
+        e.layout = s->layout; e.stream = run;
+        const md_sim saved = *s;                        // plain data: restored if the capture fails
+        const int64_t l0 = s->launches;
+        s->stream = run;
+        cudaGraph_t graph = nullptr;
+        int r = MD_OK;
+        if (cudaStreamBeginCapture(run, cudaStreamCaptureModeThreadLocal) != cudaSuccess) r = MD_ECUDA;
+        if (r == MD_OK) {
+            for (int q = 0; q < unit && r == MD_OK; q++) r = one_step(s, algo, 2, false);
+            cudaError_t ce = cudaStreamEndCapture(run, &graph);
+            if (ce != cudaSuccess || !graph) r = MD_ECUDA;
+        }
+        if (r == MD_OK && cudaGraphInstantiate(&e.exec, graph, 0) != cudaSuccess) r = MD_ECUDA;
+        if (graph) cudaGraphDestroy(graph);
+        const bool same = s->pos == saved.pos && s->vel == saved.vel && s->ap_since_sort == saved.ap_since_sort &&
+                          s->layout == saved.layout;
+        e.launches = s->launches - l0;
+        s->stream = user;
+        s->launches = l0;
+        if (r != MD_OK || !same) {
+            // nothing was executed during the capture: put the host state back and go on without graphs
+            cudaGetLastError();
+            if (e.exec) cudaGraphExecDestroy(e.exec);
+            GraphEntry keep[MD_NGRAPH];
+            memcpy(keep, s->graphs, sizeof(keep));
+            cudaStream_t cs = s->cap_stream;
+            *s = saved;
+            memcpy(s->graphs, keep, sizeof(keep));
+            s->cap_stream = cs;
+            s->use_graph = false;
+            return MD_OK;
+        }
+        if (s->graphs[victim].exec) cudaGraphExecDestroy(s->graphs[victim].exec);
+        s->graphs[victim] = e;
+        g = &s->graphs[victim];
+    }
+    g->stamp = ++s->graph_clock;
+    for (int64_t u = 0; u < nunits; u++) {
+        CK(cudaGraphLaunch(g->exec, run));
+        s->launches += g->launches;
+    }
+    s->graph_replays += nunits;
+    if (algo == MD_CELL) s->binned = false;
+    *done = nunits * unit;
+    return MD_OK;
+}
+
 extern "C" int md_compute_forces(md_sim *s, int algo)
 {
     if (!s) return MD_EINVAL;
@@ -405,15 +523,21 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
     // Inside one call the second half-kick of step k is folded into the first kernel of step
     // k + 1 (same F, separate FMAs: bit-identical velocities); only the last step runs the
     // half-kick + KE kernel, since intermediate kinetic energies are not observable.
-    for (int64_t k = 0; k < nsteps; k++) {
-        const int kicks = (k > 0) ? 2 : 1;
-        if ((r = (algo == MD_CELL) ? ljmd_kick_drift_bin(s, kicks) : ljmd_kick_drift(s, kicks))) return r;
-        ljmd_tick(s, TAG_INTEGRATE);
-        if ((r = eval_forces(s, algo))) return r;
-        if (k == nsteps - 1) {
-            if ((r = ljmd_kick_ke(s))) return r;
-            ljmd_tick(s, TAG_INTEGRATE);
+    // Interior steps (all but the first and the last) are identical launch sequences and are
+    // replayed from a CUDA graph, one unit of steps per replay.
+    int64_t k = 0;
+    while (k < nsteps) {
+        if (k > 0 && k < nsteps - 1 && s->use_graph && !s->time_kernels) {
+            const int unit = graph_unit(s, algo);
+            if (nsteps - 1 - k >= unit) {
+                int64_t done = 0;
+                if ((r = replay_interior(s, algo, unit, (nsteps - 1 - k) / unit, &done))) return r;
+                k += done;
+                if (done) continue;
+            }
         }
+        if ((r = one_step(s, algo, (k > 0) ? 2 : 1, k == nsteps - 1))) return r;
+        k++;
     }
     if ((r = ljmd_reduce_energies(s))) return r;
     ljmd_tick(s, TAG_OTHER);
@@ -451,7 +575,7 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
         if (value < 1) return MD_EINVAL;
         s->sort_every = (int)value;
     } else return MD_EINVAL;
-    for (int k = 0; k < 2; k++) s->graph_ok[k] = false;
+    drop_graphs(s);
     return MD_OK;
 }
 
@@ -463,6 +587,7 @@ extern "C" int md_get_stat(md_sim *s, const char *key, double *value)
     else if (!strcmp(key, "last_side")) *value = s->grid.last;
     else if (!strcmp(key, "kernel_launches")) *value = (double)s->launches;
     else if (!strcmp(key, "steps_done")) *value = (double)s->steps_done;
+    else if (!strcmp(key, "graph_replays")) *value = (double)s->graph_replays;
     else if (!strcmp(key, "ap_nsplit")) *value = s->ap_nsplit;
     else if (!strcmp(key, "ap_tiled")) *value = s->ap_tiled ? 1 : 0;
     else if (!strcmp(key, "ap_ntiles")) *value = s->ap_ntiles;

@@ -291,3 +291,24 @@ def test_melted_snapshot_n4000(b, oracle_uniforms):
             ke, pe, w = s.energies()
             assert pe == pytest.approx(peo, rel=E_REL[algo]) and w == pytest.approx(wo, rel=E_REL[algo])
             assert ke == pytest.approx(oracle.kinetic_energy(v.astype(np.float64)), rel=1e-9)
+
+
+@pytest.mark.parametrize("algo,opts,nsteps", [(1, (), 25), (0, (("sort_every", 2),), 31), (0, (), 64)])
+def test_graph_replay_equals_direct_launches(b, c1, algo, opts, nsteps):
+    """Interior steps replayed from a CUDA graph ("graph" = 1, default) against direct launches."""
+    out = []
+    for graph in (1, 0):
+        with b.Sim(c1["N"], c1["L"]) as s:
+            for k, v in opts + (("graph", graph),):
+                s.option(k, v)
+            s.set_state(c1["pos"], c1["vel"])
+            s.step(nsteps, algo)
+            s.step(nsteps, algo)                         # second call: cached graph, other buffer parity
+            assert (s.stat("graph_replays") > 0) == bool(graph)
+            out.append((s.get_state(), s.energies(), s.stat("kernel_launches")))
+    (p1, v1), e1, l1 = out[0]
+    (p0, v0), e0, l0 = out[1]
+    assert l1 == l0                                      # same kernels, launched or replayed
+    # the counting sort's atomic ranks make the summation order run-dependent: equal up to rounding
+    assert np.max(np.abs(p1 - p0)) < 1e-5 and np.max(np.abs(v1 - v0)) < 1e-4
+    assert e1 == pytest.approx(e0, rel=2e-6)             # the virial is the most sensitive of the three
