@@ -131,6 +131,10 @@ def time_md(b, torch, sysd, algo, steps, warmup, flush, buf):
               shifted=sysd["shifted"])
     s.set_state(sysd["pos"], sysd["vel"])
     s.step(warmup, algo)
+    # two more untimed calls of the timed shape: md_step caches its CUDA graphs per buffer parity and
+    # sort phase, and capture + instantiation is a one-time cost that does not belong in a step time
+    s.step(steps, algo)
+    s.step(steps, algo)
     torch.cuda.synchronize()
     # (1) steady state: K steps in one call, the way a user runs MD
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
