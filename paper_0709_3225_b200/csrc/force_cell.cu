@@ -1,20 +1,22 @@
 // Cell-list Lennard-Jones force.  PAPER.md:112: one block (here: one
-// warp) per cell c0, the atoms of its 27 neighbour cells staged through shared memory.
+// warp) per cell, the atoms of its 27 neighbour cells staged through shared memory.
 // What differs from the paper's G80 kernel (DESIGN.md sections 6, 7, 10):
 //   * CSR cells from the counting sort instead of 32 placeholders with virtual particles;
-//   * candidates are staged once per cell in the centre cell's frame, u = l + (offset between
-//     the two cell origins) - h, exact in FP32 on the power-of-two aligned grid;
-//   * the distance test is a FILTER, 3 FFMA + compare + ballot per (atom i, 32 candidates)
-//     row: lane = candidate (registers), the cell's atoms unrolled in registers,
+//   * a warp owns a "row group" of 1..4 consecutive cells of one z-column (1 when cells hold about
+//     13 atoms, more when they are sparsely filled); its candidates, the 9 x (cells + 2) cells
+//     around it, are staged once in the frame of the group's first cell, u = l + (offset between
+//     the cell origins) - centre, exact in FP32 on the power-of-two aligned grid;
+//   * the distance test is a FILTER, 3 FFMA + compare + ballot per (atom i, 32 candidates):
+//     lane = candidate (registers), the group's atoms two per FFMA2 in registers,
 //     r^2 - |u_i|^2 = |u_j|^2 - 2 u_i.u_j against rc^2 + margin - |u_i|^2.  The ballot is the
-//     i-major hit-mask word, stored to shared memory;
+//     i-major hit-mask word, stored to shared memory four rows per 16-byte store;
 //   * evaluation: lane = (atom i, slice of its mask words); every lane walks its own hit bits,
-//     so only the 15 % of candidates inside rc reach the pair term and the lanes stay
-//     balanced (about 26 hits each at density 0.8);
+//     two per iteration, so only the 15 % of candidates inside rc reach the pair term;
 //   * mixed precision: pairs with r^2 < precise_r2 (default 1.3 sigma^2, the steep part of the
-//     potential) are queued and evaluated in FP64 from the exact local coordinates, the rest
-//     in FP32 with a Newton-corrected reciprocal; sums of s^6 and s^12 give PE and the virial.
-// Tiles over candidates (FC_CAP per pass) and over atoms (32 per pass): any occupancy works.
+//     potential) or within 4e-6 of rc^2 are queued and evaluated in FP64 from the exact local
+//     coordinates, the rest in FP32 with a Newton-corrected reciprocal; sums of s^6 and s^12
+//     give PE and the virial.
+// Tiles over candidates (FC_CAP per pass) and over atoms (16 per pass): any occupancy works.
 #include <math.h>
 #include "common.cuh"
 #include "pair.cuh"
