@@ -193,7 +193,7 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
 #pragma unroll
                     for (int u = 0; u < 4; u++) {
                         const int c = c0 + 32 * u;
-                        l[u] = lpos[__float_as_int(sg[u].w) + t0 + min(c, cnt - 1)];
+                        l[u] = (c < cnt) ? lpos[__float_as_int(sg[u].w) + t0 + c] : make_float4(0.f, 0.f, 0.f, 0.f);
                     }
 #pragma unroll
                     for (int u = 0; u < 4; u++) {
