@@ -114,7 +114,7 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
  *                    the last) are replayed from a CUDA graph that holds one unit of steps (2 on the
  *                    cell path, 2 * sort_every on the sorted all-pairs path: the number of steps
  *                    after which the buffer roles repeat); 0 = launch every kernel directly
- *   "cell_group"     cells of one z-column handled by one warp of the cell-force kernel (1..4);
+ *   "cell_group"     cells of one z-column handled by one warp of the cell-force kernel (1..5);
  *                    0 (default) = chosen from the mean occupancy
  *   "time_kernels"   1 = record CUDA events around every phase of md_step (disables the graph);
  *                    read back with md_get_stat "t_force_ms", "t_build_ms", "t_integrate_ms",

@@ -110,6 +110,7 @@ struct md_sim {
     int forces_algo;
     bool use_graph;
     int sort_every;
+    bool precise_r2_user;         // "precise_r2" was set through md_set_option
     int cell_group;               // cells per row group of the cell-force kernel; 0 = automatic
     int64_t launches, steps_done;
     // CUDA graphs of one "unit" of interior steps (ljmd_api.cu): the unit is the number of steps after

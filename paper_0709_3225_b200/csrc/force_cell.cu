@@ -26,8 +26,10 @@
 #define FC_CAP 448                    // staged candidates per pass
 #define FC_STEPS (FC_CAP / 32)
 #define FC_CLOSE 8                    // queued FP64 pairs per lane
-#define FC_KZ_MAX 4                   // cells per row group
-#define FC_NSEG (9 * (FC_KZ_MAX + 2) + 2)
+#ifndef FC_KZ_MAX
+#define FC_KZ_MAX 5                   // cells per row group
+#endif
+#define FC_NSEG ((9 * (FC_KZ_MAX + 2) + 2 + 3) & ~3)   // multiple of 4: keeps the arrays behind it 16-byte aligned
 #ifndef FC_MINB
 #define FC_MINB 4
 #endif
@@ -452,7 +454,10 @@ int ljmd_forces_cell(md_sim *s)
     int kz = s->cell_group;
     if (kz <= 0) {
         const double occ = (double)s->N / (double)g.ncells;
-        kz = (int)(18.0 / (occ > 0.5 ? occ : 0.5) + 0.5);
+        // measured optimum (B200): one cell per warp from about 11 atoms per cell on, else about
+        // 22 filter rows per group
+        kz = (occ >= 11.0) ? 1 : (int)(22.0 / (occ > 0.5 ? occ : 0.5) + 0.5);
+        if (kz < 2 && occ < 11.0) kz = 2;
     }
     if (kz > FC_KZ_MAX) kz = FC_KZ_MAX;
     if (kz < 1 || g.n < 8) kz = 1;                  // dz * side must stay exact in FP32 (L >= 16)
@@ -466,7 +471,13 @@ int ljmd_forces_cell(md_sim *s)
     FcConst K;
     K.rc2_lo = (float)(P.rc2 * (1.0 - 4e-6));
     K.rc2_hi = (float)(P.rc2 * (1.0 + 4e-6));
-    K.p2 = (float)fmin(P.precise_r2, 3.0e38);
+    // Row groups of several cells stage candidates up to 3.5 cell sides from the frame centre, where
+    // atoms whose global coordinate is below 4 (8 for kz = 5) lose up to 2.4e-7 (4.8e-7) of their
+    // offset to FP32 rounding; the FP64 window is widened to r^2 < 1.5 sigma^2 so that every pair
+    // with |df/dr| > 5 is still evaluated from the exact coordinates.
+    double p2 = P.precise_r2;
+    if (kz > 1 && !s->precise_r2_user) p2 = fmax(p2, 1.5 * P.sig2);
+    K.p2 = (float)fmin(p2, 3.0e38);
     K.h = 0.5f * g.side;
     K.hd = (double)K.h;
     K.kz = kz;

@@ -561,6 +561,7 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
     else if (!strcmp(key, "precise_r2")) {
         if (!(value >= 0)) return MD_EINVAL;
         s->pp.precise_r2 = value;
+        s->precise_r2_user = true;
     } else if (!strcmp(key, "ap_general")) {
         s->ap_force_general = value != 0.0;
     } else if (!strcmp(key, "ap_R")) {
@@ -569,7 +570,7 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
         ljmd_ap_set_R(s, R);
         s->layout = LAYOUT_NONE;
     } else if (!strcmp(key, "cell_group")) {
-        if (value < 0 || value > 4) return MD_EINVAL;
+        if (value < 0 || value > 5) return MD_EINVAL;
         s->cell_group = (int)value;
     } else if (!strcmp(key, "sort_every")) {
         if (value < 1) return MD_EINVAL;

@@ -83,7 +83,7 @@ def test_forces_cell_tiling_and_precision_modes(b, n, rho, amp, precise_r2):
 
 
 @pytest.mark.parametrize("n,rho,amp", [(16, 0.3, 0.15), (14, 0.1, 0.3), (13, 0.8, 0.1)])
-@pytest.mark.parametrize("kz", [1, 2, 3, 4])
+@pytest.mark.parametrize("kz", [1, 2, 3, 4, 5])
 def test_forces_cell_row_groups(b, n, rho, amp, kz):
     """Row groups of kz cells per warp (option "cell_group"): same forces for every kz, including
     groups that touch the periodic seam in z and the ragged last group of a column."""
