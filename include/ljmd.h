@@ -37,7 +37,12 @@ typedef enum md_status {
     MD_EUNSUPPORTED = -6  /* valid request that this build does not implement */
 } md_status;
 
-enum { MD_ALLPAIRS = 0, MD_CELL = 1 };                       /* algo */
+/* algo.  MD_VERLET (an extension beyond the paper's two algorithms; it discusses neighbour lists in
+ * PAPER.md:100-104): neighbour lists with a skin, built from a cell list of side >= rc + skin and rebuilt,
+ * on the device's own decision, whenever an atom has moved more than skin / 2 since the last build.  Same
+ * forces as the other two paths; MD_EDOMAIN if int[L / (rc + skin)] < 3, MD_EUNSUPPORTED if N > 2^23 - 1,
+ * MD_ENOMEM from md_step if a list overflowed its capacity (1.4 x the mean length + 32). */
+enum { MD_ALLPAIRS = 0, MD_CELL = 1, MD_VERLET = 2 };
 enum { MD_TRUNCATED = 0, MD_ENERGY_SHIFTED = 1, MD_FORCE_SHIFTED = 2 }; /* shifted */
 enum { R48_U32_HI32 = 0, R48_U32_HI31 = 1, R48_F64 = 2, R48_U64_STATE = 3 }; /* kind */
 
@@ -114,6 +119,7 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
  *                    the last) are replayed from a CUDA graph that holds one unit of steps (2 on the
  *                    cell path, 2 * sort_every on the sorted all-pairs path: the number of steps
  *                    after which the buffer roles repeat); 0 = launch every kernel directly
+ *   "skin"           MD_VERLET: list radius minus rc (default 0.3 sigma); only before the first use
  *   "cell_group"     cells of one z-column handled by one warp of the cell-force kernel (1..5);
  *                    0 (default) = chosen from the mean occupancy
  *   "time_kernels"   1 = record CUDA events around every phase of md_step (disables the graph);
@@ -126,7 +132,8 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
  *   "ap_R"           atoms per thread (1, 2, 4, 8) of the sorted all-pairs kernel, overriding the
  *                    choice made from N and L; blocks too wide for the box test per-pair images
  * md_get_stat keys: "ncell" (cells per dimension), "max_occupancy", "kernel_launches"
- * (kernels launched by this handle so far, graph nodes included), "graph_replays", "steps_done",
+ * (kernels launched by this handle so far, graph nodes included), "graph_replays", "vl_builds", "vl_steps",
+ * "vl_overflow", "vl_cap" (neighbour-list builds, evaluations, overflow flag, capacity), "steps_done",
  * "side" (cell side). */
 int md_set_option(md_sim *s, const char *key, double value);
 int md_get_stat(md_sim *s, const char *key, double *value);

@@ -19,7 +19,7 @@ if not os.path.exists(LIB_PATH):
 _lib = ctypes.CDLL(LIB_PATH)
 
 MD_OK, MD_EINVAL, MD_EDOMAIN, MD_ESTATE, MD_ENOMEM, MD_ECUDA, MD_EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
-MD_ALLPAIRS, MD_CELL = 0, 1
+MD_ALLPAIRS, MD_CELL, MD_VERLET = 0, 1, 2
 MD_TRUNCATED, MD_ENERGY_SHIFTED, MD_FORCE_SHIFTED = 0, 1, 2
 R48_U32_HI32, R48_U32_HI31, R48_F64, R48_U64_STATE = 0, 1, 2, 3
 R48_DTYPES = {0: np.uint32, 1: np.uint32, 2: np.float64, 3: np.uint64}

@@ -78,8 +78,9 @@ __device__ __forceinline__ unsigned long long sc_word(unsigned long long epoch, 
 __global__ void __launch_bounds__(SC_T)
 k_scan_cells(int *__restrict__ cell_count, int *__restrict__ cell_start, int ncells,
              unsigned long long *__restrict__ max_occ, ScanCtl *__restrict__ ctl,
-             volatile unsigned long long *__restrict__ state)
+             volatile unsigned long long *__restrict__ state, const int *__restrict__ cond)
 {
+    if (cond && !*cond) return;                                // conditional launch (verlet.cu): nothing is touched
     __shared__ int wsum[SC_T / 32];
     __shared__ int s_tile, s_prefix;
     __shared__ unsigned s_base;
@@ -210,11 +211,11 @@ k_scatter(const float4 *__restrict__ pos, const float4 *__restrict__ vel, int N,
     lpos[dst] = l;
 }
 
-int ljmd_scan_counts(md_sim *s, int *count, int *start, int n)
+int ljmd_scan_counts(md_sim *s, int *count, int *start, int n, const int *cond)
 {
     const int nb = (n + SC_TILE - 1) / SC_TILE;
     if (nb > s->scan_cap) return MD_ENOMEM;
-    k_scan_cells<<<nb, SC_T, 0, s->stream>>>(count, start, n, s->max_occ, s->scan_ctl, s->scan_state);
+    k_scan_cells<<<nb, SC_T, 0, s->stream>>>(count, start, n, s->max_occ, s->scan_ctl, s->scan_state, cond);
     CKL(s);
     return MD_OK;
 }

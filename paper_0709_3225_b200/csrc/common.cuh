@@ -61,6 +61,15 @@ struct ScanCtl {
     unsigned long long epoch;     // launch number (30 bits), tags the look-back words and max_occ
 };
 
+// Device-side control block of the neighbour-list path (verlet.cu)
+struct VlCtl {
+    unsigned maxd2;               // bits of the largest squared displacement since the last build
+    int rebuild;                  // this step's decision (read by the build kernels)
+    int force;                    // host request: build at the next evaluation
+    int overflow;                 // some list was longer than the capacity
+    int nbuilds, nsteps;          // statistics
+};
+
 enum { TAG_START = -1, TAG_INTEGRATE = 0, TAG_BUILD = 1, TAG_FORCE = 2, TAG_OTHER = 3, TAG_FORCE2 = 4, TAG_COUNT = 5 };
 
 struct md_sim {
@@ -70,6 +79,13 @@ struct md_sim {
     float Lf, dtf, hdtf;
     PairParams pp;
     Grid grid;            // grid.n == 0 when the box has fewer than 3 cells per dimension
+    Grid vgrid;           // cells of side >= rc + skin for the neighbour-list path (n == 0: unavailable)
+    double skin;
+    unsigned *vl_list;    // [vl_cap][vl_npad] slot of j | offset index << 23
+    int *vl_count;        // [N]
+    float4 *vl_lbuild;    // [N] local coordinates at the last build
+    VlCtl *vl_ctl;
+    int vl_cap, vl_npad;
     int grid_paper_n;     // int[L/rc]
     cudaStream_t stream;
 
@@ -128,7 +144,7 @@ struct md_sim {
     int64_t n_phase[TAG_COUNT];
 };
 
-enum { LAYOUT_NONE = 0, LAYOUT_CELL = 1, LAYOUT_TILE = 2 };
+enum { LAYOUT_NONE = 0, LAYOUT_CELL = 1, LAYOUT_TILE = 2, LAYOUT_VERLET = 3 };
 // Record an event; the time since the previous tick is attributed to `tag`.
 void ljmd_tick(md_sim *s, int tag);
 int ljmd_collect_ticks(md_sim *s);
@@ -144,7 +160,10 @@ int ljmd_reduce_energies(md_sim *s);
 int ljmd_forces_allpairs(md_sim *s);
 void ljmd_ap_plan(md_sim *s);
 void ljmd_ap_set_R(md_sim *s, int R);                       // R in {0 (general kernel), 1, 2, 4, 8}
-int ljmd_scan_counts(md_sim *s, int *count, int *start, int n);   // exclusive scan, zeroes count
+int ljmd_scan_counts(md_sim *s, int *count, int *start, int n, const int *cond = nullptr);   // exclusive scan, zeroes count; cond: device flag, 0 = do nothing
+int ljmd_vl_kick_drift(md_sim *s, int kicks);
+int ljmd_forces_verlet(md_sim *s);
+int ljmd_vl_stats(md_sim *s, int *nbuilds, int *nsteps, int *overflow);
 int ljmd_cell_build(md_sim *s);
 int ljmd_forces_cell(md_sim *s);
 

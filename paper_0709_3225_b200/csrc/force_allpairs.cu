@@ -631,7 +631,7 @@ int ljmd_forces_allpairs(md_sim *s)
                                                               jchunk, s->fpart, ppe, pw);
         CKL(s);
         s->n_pe = niblk * nsplit;
-        if (s->layout == LAYOUT_CELL) s->layout = LAYOUT_NONE;      // lpos no longer tracked
+        if (s->layout == LAYOUT_CELL || s->layout == LAYOUT_VERLET) s->layout = LAYOUT_NONE;   // lpos no longer tracked
         ljmd_tick(s, TAG_FORCE);
         k_combine_forces<<<(N + 255) / 256, 256, 0, s->stream>>>(s->frc, s->fpart, N, nsplit);
         CKL(s);

@@ -68,17 +68,15 @@ void ljmd_dev_free(void *p, cudaStream_t st)
 // ---- grid and pair constants ----------------------------------------------------------
 // Cells on a lattice whose spacing is a multiple of g = ulp of the binade of L, so that cell
 // origins c*side are exact floats and x - origin is exact.
-static void setup_grid(md_sim *s)
+static void make_grid(const md_sim *s, double rc, Grid &g)
 {
-    double L = s->L, rc = s->rc;
-    s->grid_paper_n = (int)floor(L / rc);
-    Grid &g = s->grid;
+    double L = s->L;
     memset(&g, 0, sizeof(g));
     g.L = s->Lf;
     int e;
     frexp(L, &e);                                    // L = m 2^e, m in [0.5,1)
     double q = ldexp(1.0, e - 24);                   // ulp of floats in [2^(e-1), 2^e)
-    int n = s->grid_paper_n;
+    int n = (int)floor(L / rc);
     if (n > 1023) n = 1023;                          // cell id must fit 30 bits
     double side = 0.0;
     for (; n >= 3; n--) {
@@ -91,6 +89,13 @@ static void setup_grid(md_sim *s)
     g.side = (float)side;
     g.last = (float)(L - (n - 1) * side);
     g.inv_side = (float)(1.0 / side);
+}
+
+static void setup_grid(md_sim *s)
+{
+    s->grid_paper_n = (int)floor(s->L / s->rc);
+    make_grid(s, s->rc, s->grid);
+    make_grid(s, s->rc + s->skin, s->vgrid);         // neighbour-list path: cells of side >= rc + skin
 }
 
 static void setup_pair(md_sim *s)
@@ -175,7 +180,7 @@ static void free_all(md_sim *s)
     free(s->ev_pool);
     free(s->ev_tag);
     void *ptrs[] = {s->pos, s->vel, s->frc, s->pos2, s->vel2, s->lpos, s->cell_of, s->rank, s->cell_count,
-                    s->cell_start, s->max_occ, s->scan_ctl, s->scan_state, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list,
+                    s->cell_start, s->max_occ, s->scan_ctl, s->scan_state, s->vl_list, s->vl_count, s->vl_lbuild, s->vl_ctl, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list,
                     s->tile_start};
     for (void *p : ptrs) ljmd_dev_free(p, st);
 }
@@ -208,6 +213,7 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->hdtf = (float)(0.5 * dt);
     s->use_graph = true;
     s->sort_every = 10;
+    s->skin = 0.3 * sigma;
     setup_grid(s);
     setup_pair(s);
 
@@ -371,15 +377,18 @@ extern "C" int md_get_energies(md_sim *s, double *KE, double *PE, double *W)
 // ---- force evaluation and stepping ------------------------------------------------------
 static int check_algo(md_sim *s, int algo)
 {
-    if (algo != MD_ALLPAIRS && algo != MD_CELL) return MD_EINVAL;
+    if (algo != MD_ALLPAIRS && algo != MD_CELL && algo != MD_VERLET) return MD_EINVAL;
     if (algo == MD_CELL && (s->grid_paper_n < 3 || s->grid.n < 3)) return MD_EDOMAIN;
+    if (algo == MD_VERLET && s->vgrid.n < 3) return MD_EDOMAIN;
     return MD_OK;
 }
 
 static int eval_forces(md_sim *s, int algo)
 {
     int r;
-    if (algo == MD_CELL) {
+    if (algo == MD_VERLET) {
+        if ((r = ljmd_forces_verlet(s))) return r;
+    } else if (algo == MD_CELL) {
         if ((r = ljmd_cell_build(s))) return r;
         ljmd_tick(s, TAG_BUILD);
         if ((r = ljmd_forces_cell(s))) return r;
@@ -394,7 +403,9 @@ static int eval_forces(md_sim *s, int algo)
 static int one_step(md_sim *s, int algo, int kicks, bool last)
 {
     int r;
-    if ((r = (algo == MD_CELL) ? ljmd_kick_drift_bin(s, kicks) : ljmd_kick_drift(s, kicks))) return r;
+    if ((r = (algo == MD_CELL) ? ljmd_kick_drift_bin(s, kicks)
+                               : (algo == MD_VERLET) ? ljmd_vl_kick_drift(s, kicks) : ljmd_kick_drift(s, kicks)))
+        return r;
     ljmd_tick(s, TAG_INTEGRATE);
     if ((r = eval_forces(s, algo))) return r;
     if (last) {
@@ -409,6 +420,7 @@ static int one_step(md_sim *s, int algo, int kicks, bool last)
 static int graph_unit(const md_sim *s, int algo)
 {
     if (algo == MD_CELL) return 2;
+    if (algo == MD_VERLET) return 1;                  // no buffer swaps: builds are decided and done on the device
     if (s->ap_tiled && !s->ap_force_general) return 2 * s->sort_every;
     return 1;
 }
@@ -513,7 +525,9 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
     if (!s->has_state) return MD_ESTATE;
     int r = check_algo(s, algo);
     if (r) return r;
-    if (!s->forces_valid) {
+    // the neighbour-list integrator needs the lists' local coordinates: evaluate first if another
+    // path (or md_set_state) ran last
+    if (!s->forces_valid || (algo == MD_VERLET && s->layout != LAYOUT_VERLET && nsteps > 0)) {
         if ((r = eval_forces(s, algo))) return r;
         if ((r = ljmd_ke_only(s))) return r;
         s->forces_valid = true;
@@ -543,6 +557,11 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
     ljmd_tick(s, TAG_OTHER);
     if ((r = ljmd_collect_ticks(s))) return r;
     CK(cudaStreamSynchronize(s->stream));
+    if (algo == MD_VERLET) {
+        int nb, ns, ovf;
+        if ((r = ljmd_vl_stats(s, &nb, &ns, &ovf))) return r;
+        if (ovf) return MD_ENOMEM;                      // a neighbour list overflowed: results are not valid
+    }
     s->forces_algo = algo;
     s->steps_done += nsteps;
     return MD_OK;
@@ -569,6 +588,10 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
         if (R != 1 && R != 2 && R != 4 && R != 8) return MD_EINVAL;
         ljmd_ap_set_R(s, R);
         s->layout = LAYOUT_NONE;
+    } else if (!strcmp(key, "skin")) {
+        if (!(value > 0) || s->vl_list) return MD_EINVAL;          // before the first use of MD_VERLET
+        s->skin = value;
+        setup_grid(s);
     } else if (!strcmp(key, "cell_group")) {
         if (value < 0 || value > 5) return MD_EINVAL;
         s->cell_group = (int)value;
@@ -589,6 +612,11 @@ extern "C" int md_get_stat(md_sim *s, const char *key, double *value)
     else if (!strcmp(key, "kernel_launches")) *value = (double)s->launches;
     else if (!strcmp(key, "steps_done")) *value = (double)s->steps_done;
     else if (!strcmp(key, "graph_replays")) *value = (double)s->graph_replays;
+    else if (!strcmp(key, "vl_builds") || !strcmp(key, "vl_steps") || !strcmp(key, "vl_overflow")) {
+        int nb, ns, ovf, r = ljmd_vl_stats(s, &nb, &ns, &ovf);
+        if (r) return r;
+        *value = !strcmp(key, "vl_builds") ? nb : !strcmp(key, "vl_steps") ? ns : ovf;
+    } else if (!strcmp(key, "vl_cap")) *value = s->vl_cap;
     else if (!strcmp(key, "ap_nsplit")) *value = s->ap_nsplit;
     else if (!strcmp(key, "ap_tiled")) *value = s->ap_tiled ? 1 : 0;
     else if (!strcmp(key, "ap_ntiles")) *value = s->ap_ntiles;

@@ -1,0 +1,147 @@
+"""The neighbour-list path (algo = MD_VERLET) against the FP64 oracle and against
+the cell path (gpu-marked).  Same tolerances as the other two force paths (R15, R17)."""
+import numpy as np
+import pytest
+
+import oracle
+from helpers import force_check
+from paper_0709_3225_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def b():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_0709_3225_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def c1(oracle_uniforms):
+    return wl.md_system("c1_allpairs_500", oracle_uniforms)
+
+
+@pytest.mark.parametrize("n,rho,amp", [(5, 0.8, 0.10), (6, 0.8, 0.10), (7, 0.9, 0.08), (5, 0.3, 0.15), (10, 0.8, 0.1),
+                                       (8, 0.05, 0.3), (6, 1.3, 0.06)])
+@pytest.mark.parametrize("shifted", [0, 1, 2])
+def test_forces_match_oracle(b, n, rho, amp, shifted):
+    pos, L = wl.perturbed_fcc(n, rho, amp, seed=300 + n)
+    vel = np.zeros_like(pos)
+    with b.Sim(pos.shape[0], L, shifted=shifted) as s:
+        s.set_state(pos, vel)
+        s.compute_forces(b.MD_VERLET)
+        F, (ke, pe, w) = s.forces(), s.energies()
+    Fo, peo, wo = oracle.forces(pos.astype(np.float64), L, mode=shifted, algo=0)
+    nviol, worst = force_check(F, Fo)
+    assert nviol == 0, (nviol, worst)
+    assert pe == pytest.approx(peo, rel=1e-6) and w == pytest.approx(wo, rel=1e-6)
+
+
+def test_config1_energy_trace_and_list_reuse(b, c1):
+    """Per-step total energy within 1e-5 of the oracle over 100 steps (R17) while the lists are reused."""
+    _, _, _, tr = oracle.verlet_run(c1["pos"], c1["vel"], c1["L"], 100, algo=0)
+    with b.Sim(c1["N"], c1["L"]) as s:
+        s.set_state(c1["pos"], c1["vel"])
+        s.compute_forces(b.MD_VERLET)
+        worst = 0.0
+        for t in range(101):
+            if t:
+                s.step(1, b.MD_VERLET)
+            ke, pe, w = s.energies()
+            Eo = tr[t, 0] + tr[t, 1]
+            worst = max(worst, abs(ke + pe - Eo) / abs(Eo))
+        assert worst < 1e-5, worst
+        builds, evals = s.stat("vl_builds"), s.stat("vl_steps")
+        assert evals == 101 and 3 <= builds <= 40, (builds, evals)       # reused, and rebuilt when atoms moved
+        p, v = s.get_state()
+        F = s.forces()
+        Fo, _, _ = oracle.forces(p.astype(np.float64), c1["L"], algo=0)
+        assert force_check(F, Fo)[0] == 0                                 # forces from a list several steps old
+
+
+def test_multi_step_and_graph_equal_single_steps_and_cell_path(b, c1):
+    out = []
+    for algo, chunks, graph in ((b.MD_VERLET, [60], 1), (b.MD_VERLET, [1] * 60, 1), (b.MD_VERLET, [60], 0), (b.MD_CELL, [60], 1)):
+        with b.Sim(c1["N"], c1["L"]) as s:
+            s.option("graph", graph)
+            s.set_state(c1["pos"], c1["vel"])
+            for c in chunks:
+                s.step(c, algo)
+            out.append((s.get_state(), s.energies()))
+    for (p, v), e in out[1:]:
+        d = p - out[0][0][0]
+        d -= c1["L"] * np.rint(d / c1["L"])
+        assert np.max(np.abs(d)) < 2e-5 and np.max(np.abs(v - out[0][0][1])) < 2e-4
+        assert e[0] + e[1] == pytest.approx(out[0][1][0] + out[0][1][1], rel=1e-6)
+
+
+def test_switching_paths_between_calls(b, c1):
+    with b.Sim(c1["N"], c1["L"]) as s:
+        s.set_state(c1["pos"], c1["vel"])
+        s.step(15, b.MD_VERLET)
+        s.step(7, b.MD_CELL)
+        s.step(9, b.MD_ALLPAIRS)
+        s.step(15, b.MD_VERLET)
+        p, v = s.get_state()
+        F = s.forces()
+        ke, pe, w = s.energies()
+    Fo, peo, wo = oracle.forces(p.astype(np.float64), c1["L"], algo=0)
+    assert force_check(F, Fo)[0] == 0 and pe == pytest.approx(peo, rel=1e-6)
+
+
+def test_skin_option_and_domain_errors(b):
+    pos, L = wl.perturbed_fcc(6, 0.8, 0.1, seed=3)
+    Fo, _, _ = oracle.forces(pos.astype(np.float64), L, algo=0)
+    for skin in (0.1, 0.6):
+        with b.Sim(pos.shape[0], L) as s:
+            s.option("skin", skin)
+            s.set_state(pos, np.zeros_like(pos))
+            s.compute_forces(b.MD_VERLET)
+            assert force_check(s.forces(), Fo)[0] == 0
+            with pytest.raises(b.MDError):
+                s.option("skin", 0.2)                  # lists exist
+    with b.Sim(100, 8.0) as s:                         # int[8 / 2.8] = 2 cells: no neighbour-list path
+        s.set_state(np.random.default_rng(1).random((100, 3)).astype(np.float32) * 8, np.zeros((100, 3), np.float32))
+        with pytest.raises(b.MDError) as e:
+            s.compute_forces(b.MD_VERLET)
+        assert e.value.code == b.MD_EDOMAIN
+
+
+def test_list_overflow_is_reported(b):
+    """600 atoms inside one cell of a sparse box: lists far longer than the capacity -> MD_ENOMEM, never silently dropped."""
+    g = np.stack(np.meshgrid(np.arange(10), np.arange(10), np.arange(6), indexing="ij"), -1).reshape(-1, 3)
+    pos = (15.2 + 0.24 * g).astype(np.float32)
+    with b.Sim(pos.shape[0], 30.5) as s:
+        s.set_state(pos, np.zeros_like(pos))
+        s.compute_forces(b.MD_VERLET)
+        assert s.stat("vl_overflow") == 1
+        with pytest.raises(b.MDError) as e:
+            s.step(1, b.MD_VERLET)
+        assert e.value.code == b.MD_ENOMEM
+
+
+@pytest.mark.parametrize("name,steps", [("c3_cell_256k", 100), ("c4a_cell_2048k", 40), ("c4b_cell_2048k_rho03", 40)])
+def test_full_size_parity(b, name, steps):
+    import os
+    oracle.set_threads(os.cpu_count() or 1)
+
+    def src(seed48, n):
+        out, _ = b.rand48([seed48], n, b.R48_F64)
+        return out[0]
+    sysd = wl.md_system(name, src)
+    with b.Sim(sysd["N"], sysd["L"]) as s:
+        s.set_state(sysd["pos"], sysd["vel"])
+        s.step(steps, b.MD_VERLET)
+        ke, pe, w = s.energies()
+        F = s.forces()
+        p, v = s.get_state()
+        assert s.stat("vl_builds") < s.stat("vl_steps")
+    Fo, peo, wo = oracle.forces(p.astype(np.float64), sysd["L"], algo=1)
+    tol = np.maximum(1e-4 * np.abs(Fo), 1e-5)
+    bad = np.argwhere(np.abs(F.astype(np.float64) - Fo) > tol)
+    assert len(bad) <= 8, len(bad)                     # at most a few R16 (cutoff-window) pairs at this size
+    for a, c in bad:
+        assert abs(F[a, c] - Fo[a, c]) < 0.04 + 1e-4
+    assert pe == pytest.approx(peo, rel=1e-6) and w == pytest.approx(wo, rel=1e-6)
