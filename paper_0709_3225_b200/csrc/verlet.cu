@@ -218,7 +218,7 @@ __device__ __forceinline__ void vl_precise(const float4 *__restrict__ lpos, cons
 }
 
 template <bool MODE2>
-__global__ void __launch_bounds__(VL_T)
+__global__ void __launch_bounds__(VL_T, 8)
 k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams P, VlConst K,
            const unsigned *__restrict__ list, const int *__restrict__ count, float4 *__restrict__ frc,
            double *__restrict__ part_pe, double *__restrict__ part_w)
@@ -238,41 +238,62 @@ k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams 
         const int cnt = count[i];
         float fx = 0.f, fy = 0.f, fz = 0.f, sA = 0.f, sB = 0.f, sR = 0.f;
         int nin = 0, nq = 0;
-        double dfx = 0.0, dfy = 0.0, dfz = 0.0, dpe = 0.0, dw = 0.0;
         const unsigned *row = list + i;
-#pragma unroll 2
-        for (int k = 0; k < cnt; k++) {
-            const unsigned e = row[(size_t)k * npad];
-            const float4 lj = lpos[e & VL_JMASK];
-            const float4 o = offt[e >> 23];
-            const float dx = (lj.x - li.x) + o.x, dy = (lj.y - li.y) + o.y, dz = (lj.z - li.z) + o.z;
-            const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-            // p2 <= r2 < rc2_lo: FP32 term; the steep part and the sliver around rc^2: FP64 (queued)
-            const bool fast = r2 >= K.p2 && r2 < K.rc2_lo;
-            if (!fast && r2 < K.rc2_hi) {
-                if (nq < VL_Q) queue[nq++][threadIdx.x] = e;
-                else vl_precise(lpos, offt, P, li, e, dfx, dfy, dfz, dpe, dw);      // queue full
+        // four list entries per iteration: the coalesced list reads and the four gathers are all
+        // issued before the first pair term (the kernel is bound by the latency of the gathers)
+        for (int k = 0; k < cnt; k += 4) {
+            unsigned e[4];
+            float4 lj[4];
+#pragma unroll
+            for (int u = 0; u < 4; u++) e[u] = (k + u < cnt) ? row[(size_t)(k + u) * npad] : (unsigned)i;
+#pragma unroll
+            for (int u = 0; u < 4; u++) lj[u] = lpos[e[u] & VL_JMASK];
+#pragma unroll
+            for (int u = 0; u < 4; u++) {
+                const float4 o = offt[e[u] >> 23];
+                const float dx = (lj[u].x - li.x) + o.x, dy = (lj[u].y - li.y) + o.y, dz = (lj[u].z - li.z) + o.z;
+                float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                r2 = (k + u < cnt) ? r2 : 3.0e38f;                      // padding slot: contributes nothing
+                // p2 <= r2 < rc2_lo: FP32 term; the steep part and the sliver around rc^2: FP64 (queued)
+                const bool fast = r2 >= K.p2 && r2 < K.rc2_lo;
+                if (!fast && r2 < K.rc2_hi) {
+                    queue[min(nq, VL_Q - 1)][threadIdx.x] = e[u];
+                    nq++;
+                }
+                float inv;
+                asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(r2));
+                inv = fmaf(inv, fmaf(-r2, inv, 1.f), inv);
+                const float s2 = K.sig2 * inv;
+                float s6 = s2 * s2 * s2;
+                s6 = fast ? s6 : 0.f;
+                float fr = inv * s6 * fmaf(K.eps48, s6, -K.eps24);
+                if (MODE2) {
+                    const float r = sqrtf(r2);
+                    fr -= fast ? P.f_rcf * inv * r : 0.f;
+                    sR += fast ? (r - P.rcf) : 0.f;
+                }
+                fx = fmaf(-fr, dx, fx);
+                fy = fmaf(-fr, dy, fy);
+                fz = fmaf(-fr, dz, fz);
+                sA = fmaf(s6, s6, sA);
+                sB += s6;
+                nin += fast ? 1 : 0;
             }
-            float inv;
-            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(r2));
-            inv = fmaf(inv, fmaf(-r2, inv, 1.f), inv);
-            const float s2 = K.sig2 * inv;
-            float s6 = s2 * s2 * s2;
-            s6 = fast ? s6 : 0.f;
-            float fr = inv * s6 * fmaf(K.eps48, s6, -K.eps24);
-            if (MODE2) {
-                const float r = sqrtf(r2);
-                fr -= fast ? P.f_rcf * inv * r : 0.f;
-                sR += fast ? (r - P.rcf) : 0.f;
-            }
-            fx = fmaf(-fr, dx, fx);
-            fy = fmaf(-fr, dy, fy);
-            fz = fmaf(-fr, dz, fz);
-            sA = fmaf(s6, s6, sA);
-            sB += s6;
-            nin += fast ? 1 : 0;
         }
-        for (int q = 0; q < nq; q++) vl_precise(lpos, offt, P, li, queue[q][threadIdx.x], dfx, dfy, dfz, dpe, dw);
+        // FP64 part: the queued pairs; a thread whose queue overflowed rescans its list instead
+        double dfx = 0.0, dfy = 0.0, dfz = 0.0, dpe = 0.0, dw = 0.0;
+        if (nq <= VL_Q) {
+            for (int q = 0; q < nq; q++) vl_precise(lpos, offt, P, li, queue[q][threadIdx.x], dfx, dfy, dfz, dpe, dw);
+        } else {
+            for (int k = 0; k < cnt; k++) {
+                const unsigned e = row[(size_t)k * npad];
+                const float4 lj = lpos[e & VL_JMASK];
+                const float4 o = offt[e >> 23];
+                const float dx = (lj.x - li.x) + o.x, dy = (lj.y - li.y) + o.y, dz = (lj.z - li.z) + o.z;
+                const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                if (!(r2 >= K.p2 && r2 < K.rc2_lo) && r2 < K.rc2_hi) vl_precise(lpos, offt, P, li, e, dfx, dfy, dfz, dpe, dw);
+            }
+        }
         frc[i] = make_float4((float)(dfx + (double)fx), (float)(dfy + (double)fy), (float)(dfz + (double)fz), 0.f);
         pe = dpe + P.eps4 * ((double)sA - (double)sB) - (double)nin * P.ushift;
         w = dw + P.eps24 * (2.0 * (double)sA - (double)sB);
