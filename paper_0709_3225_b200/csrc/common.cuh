@@ -86,6 +86,7 @@ struct md_sim {
     float4 *vl_lbuild;    // [N] local coordinates at the last build
     VlCtl *vl_ctl;
     int vl_cap, vl_npad;
+    bool vl_naive_build;  // option "vl_naive_build": thread-per-atom list kernel instead of the warp filter
     int grid_paper_n;     // int[L/rc]
     cudaStream_t stream;
 
@@ -162,6 +163,7 @@ void ljmd_ap_plan(md_sim *s);
 void ljmd_ap_set_R(md_sim *s, int R);                       // R in {0 (general kernel), 1, 2, 4, 8}
 int ljmd_scan_counts(md_sim *s, int *count, int *start, int n, const int *cond = nullptr);   // exclusive scan, zeroes count; cond: device flag, 0 = do nothing
 int ljmd_vl_kick_drift(md_sim *s, int kicks);
+int ljmd_vl_build_lists(md_sim *s, const int *cond);    // force_cell.cu: lists through the cell kernel's filter
 int ljmd_forces_verlet(md_sim *s);
 int ljmd_vl_stats(md_sim *s, int *nbuilds, int *nsteps, int *overflow);
 int ljmd_cell_build(md_sim *s);

@@ -23,7 +23,7 @@
 
 #define FC_WARPS 4
 #define FC_T (FC_WARPS * 32)
-#define FC_CAP 448                    // staged candidates per pass
+#define FC_CAP 544                    // staged candidates per pass (27 list cells of 18.5 atoms fit)
 #define FC_STEPS (FC_CAP / 32)
 #define FC_CLOSE 8                    // queued FP64 pairs per lane
 #ifndef FC_KZ_MAX
@@ -43,6 +43,7 @@ struct FcWarp {
     float4 seg[FC_NSEG];              // per segment (neighbour cell): origin offset minus h (x, y, z) and, as int
                                       // bits, (first slot - candidates before the cell)
     int seg_pref[FC_NSEG];            // candidates before segment k; [nseg ..] = total
+    int seg_code[FC_NSEG];            // list mode: x/y offset code (kx + 5 ky) | (dz + 1) << 8 of segment k
     float rax[16], ray[16], raz[16], rT[16];   // filter rows: -2 u_i and threshold - |u_i|^2
 };
 
@@ -52,11 +53,19 @@ struct FcConst {
     int kz, nzu;                      // cells per row group, row groups per z-column
 };
 
+struct FcList {                       // neighbour-list output of the list mode (verlet.cu)
+    unsigned *list;                   // [cap][npad]: slot of j | offset-table index << 23
+    int *count;                       // [N]
+    int *overflow;                    // set when a list is longer than cap
+    int npad, cap;
+};
+
 struct FcGroup {                      // one warp's row group
     int ibeg, ni, total, kk, cfirst;  // first slot, atoms, candidates, cells, first cell
     float hz, side;                   // z centre of the group in the frame of its first cell
     double hzd;
     int pref0, cnt0, pref1, cnt1;     // this lane's two segments (lane, lane + 32)
+    int z0, n;                        // first cell's z index, cells per dimension (list mode)
 };
 
 // z offset of row atom `slot` inside the group: (its cell - first cell) * side, exact
@@ -131,10 +140,13 @@ __device__ __forceinline__ void fc_filter(FcWarp &S, const int nsteps, const int
     }
 }
 
-template <bool MODE2>
+// LIST = true: no pair terms; every filter hit (r^2 below K.rc2_hi + margin, set to the list radius) is
+// written to the neighbour list of its row atom instead.
+template <bool MODE2, bool LIST>
 __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lpos,
                                         const int *__restrict__ cell_start, const FcGroup &G, const PairParams &P,
-                                        const FcConst &K, float4 *__restrict__ frc, double &pe_tot, double &w_tot)
+                                        const FcConst &K, float4 *__restrict__ frc, double &pe_tot, double &w_tot,
+                                        const FcList &LO)
 {
     const int lane = threadIdx.x & 31;
     const int ibeg = G.ibeg, ni = G.ni, total = G.total;
@@ -151,6 +163,10 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
         const float zoff_me = fc_row_zoff(cell_start, G, ibeg + i0 + li_);
         const float ux = lme.x - K.h, uy = lme.y - K.h, uz = (lme.z + zoff_me) - G.hz;
         const double zme = G.hzd - (double)zoff_me;
+        int rowbase = 0;                                   // list mode: entries of my atom written so far
+        int qme = 0;                                       // list mode: my cell's index inside the group
+        if (LIST)
+            for (int k = 1; k < G.kk; k++) qme += (ibeg + i0 + li_ >= cell_start[G.cfirst + k]) ? 1 : 0;
         double tx = 0.0, ty = 0.0, tz = 0.0, pe = 0.0, w = 0.0;      // this lane's totals over the passes
         // rows of the filter for this pass (lane r < 16 prepares row r)
         __syncwarp();
@@ -223,6 +239,50 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
                 if (cs >= 0 && cs < cnt) S.msk[cs >> 5][lane] &= ~(1u << (cs & 31));
             }
             __syncwarp();
+            if (LIST) {
+                // ---- list mode: count my hits, place my slice behind the lower slices of my atom, write
+                int myhits = 0;
+                if (myvalid)
+                    for (int st = sl; st < nsteps; st += SL) myhits += __popc(S.msk[st][li_]);
+                int before = 0, rowtot = 0;
+                for (int k = 0; k < SL; k++) {
+                    const int h = __shfl_sync(FULLMASK, myhits, li_ + k * nrow);
+                    before += (k < sl) ? h : 0;
+                    rowtot += h;
+                }
+                if (myvalid) {
+                    const int zr = G.z0 + qme;                                  // my cell's z index
+                    const bool top_me = zr == G.n - 1, below_top = ((zr == 0) ? G.n - 1 : zr - 1) == G.n - 1;
+                    int pos = rowbase + before;
+                    unsigned *out = LO.list + (ibeg + i0 + li_);
+                    // every lane runs through its own words at its own pace (one hit per iteration)
+                    int st = sl;
+                    unsigned m = (st < nsteps) ? S.msk[st][li_] : 0u;
+                    while (st < nsteps) {
+                        if (m == 0u) {
+                            st += SL;
+                            if (st < nsteps) m = S.msk[st][li_];
+                            continue;
+                        }
+                        const int b = fc_top_bit(m);
+                        m ^= 1u << b;
+                        const int c = st * 32 + b;
+                        const int lab = __float_as_int(S.tile[c].w) & 63;
+                        const int code = S.seg_code[lab];
+                        const int dzr = (code >> 8) - 1 - qme;                    // candidate's cell minus mine, in z
+                        const int kzc = (dzr == 0) ? 0 : (dzr > 0 ? (top_me ? 3 : 1) : (below_top ? 4 : 2));
+                        const int j = __float_as_int(S.seg[lab].w) + t0 + c;
+                        // cells two apart in z are farther than the list radius (cell side >= radius + 1e-3):
+                        // such a hit cannot occur; if it did, a self entry offset by a cell diagonal is inert
+                        unsigned e = (unsigned)j | ((unsigned)((code & 255) + 25 * kzc) << 23);
+                        if (dzr < -1 || dzr > 1) e = (unsigned)(ibeg + i0 + li_) | (31u << 23);
+                        if (pos < LO.cap) out[(size_t)pos * LO.npad] = e;
+                        pos++;
+                    }
+                }
+                rowbase += rowtot;
+                continue;
+            }
             // ---- evaluation: lane = (atom li_, slice sl) walks the hit bits of its own mask words
             // st = sl, sl + SL, ..., two hits per iteration (independent chains hide the LDS and
             // MUFU latencies); an empty word costs the lane one idle iteration.
@@ -339,6 +399,13 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
                 w -= P.f_rc * ((double)sR + (double)nin * P.rc);
             }
         }
+        if (LIST) {
+            if (sl == 0) {
+                LO.count[ibeg + i0 + li_] = min(rowbase, LO.cap);
+                if (rowbase > LO.cap) *LO.overflow = 1;
+            }
+            continue;
+        }
         // ---- reduce over the slices, store
         double ox = 0.0, oy = 0.0, oz = 0.0;               // totals of the other slices of my atom
         for (int k = 1; k < SL; k++) {
@@ -359,12 +426,13 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
 // kz > 1 packs sparsely filled cells into one set of filter rows.  The candidates are the
 // 9 columns x (kk + 2) cells around the group, i.e. the union of its cells' 27 neighbours.
 // grid = (ceil(nzu / FC_WARPS), n, n): blockIdx.z = cx, blockIdx.y = cy.
-template <bool MODE2>
+template <bool MODE2, bool LIST>
 __global__ void __launch_bounds__(FC_T, FC_MINB)
 k_force_cell_warp(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, Grid g,
                   PairParams P, FcConst K, float4 *__restrict__ frc, double *__restrict__ part_pe,
-                  double *__restrict__ part_w)
+                  double *__restrict__ part_w, FcList LO, const int *__restrict__ cond)
 {
+    if (LIST && cond && !*cond) return;                         // conditional launch (verlet.cu)
     __shared__ FcWarp sm[FC_WARPS];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int zu = blockIdx.x * FC_WARPS + wid;
@@ -402,6 +470,11 @@ k_force_cell_warp(const float4 *__restrict__ lpos, const int *__restrict__ cell_
                     const int nb = (nx * n + ny) * n + nz;
                     start[h] = cell_start[nb];
                     cnt[h] = cell_start[nb + 1] - start[h];
+                    if (LIST) {
+                        const int kx = (ax == 0) ? 0 : (ax > 0 ? ((cx == n - 1) ? 3 : 1) : ((nx == n - 1) ? 4 : 2));
+                        const int ky = (ay == 0) ? 0 : (ay > 0 ? ((cy == n - 1) ? 3 : 1) : ((ny == n - 1) ? 4 : 2));
+                        S.seg_code[sgi] = (kx + 5 * ky) | ((dz + 1) << 8);
+                    }
                 }
             }
             int carry = 0;
@@ -435,9 +508,11 @@ k_force_cell_warp(const float4 *__restrict__ lpos, const int *__restrict__ cell_
             G.ibeg = ibeg; G.ni = ni; G.total = total; G.kk = kk; G.cfirst = cfirst;
             G.hz = hz; G.hzd = (double)hz; G.side = g.side;
             G.pref0 = incl[0] - cnt[0]; G.cnt0 = cnt[0]; G.pref1 = incl[1] - cnt[1]; G.cnt1 = cnt[1];
-            fc_cell<MODE2>(S, lpos, cell_start, G, P, K, frc, pe, w);
+            G.z0 = z0; G.n = n;
+            fc_cell<MODE2, LIST>(S, lpos, cell_start, G, P, K, frc, pe, w, LO);
         }
     }
+    if (LIST) return;
     pe = warp_sum(pe);
     w = warp_sum(w);
     if (lane == 0) {
@@ -489,12 +564,50 @@ int ljmd_forces_cell(md_sim *s)
     K.sig2 = P.sig2f;
     K.eps24 = P.eps24f;
     K.eps48 = 2.0f * P.eps24f;
+    FcList none;
+    memset(&none, 0, sizeof(none));
     if (P.mode == 2)
-        k_force_cell_warp<true><<<grid, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, g, P, K, s->frc, ppe, pw);
+        k_force_cell_warp<true, false><<<grid, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, g, P, K, s->frc, ppe, pw, none, nullptr);
     else
-        k_force_cell_warp<false><<<grid, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, g, P, K, s->frc, ppe, pw);
+        k_force_cell_warp<false, false><<<grid, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, g, P, K, s->frc, ppe, pw, none, nullptr);
     CKL(s);
     ljmd_tick(s, TAG_FORCE);
     s->n_pe = (int)nunits;
+    return MD_OK;
+}
+
+// Neighbour lists (verlet.cu) through the same staging and ballot filter: cells of s->vgrid, every pair
+// inside the list radius rc + skin is written instead of evaluated.  `cond`: device flag, 0 = return at once.
+int ljmd_vl_build_lists(md_sim *s, const int *cond)
+{
+    const Grid &g = s->vgrid;
+    int kz = s->cell_group;
+    if (kz <= 0) {
+        const double occ = (double)s->N / (double)g.ncells;
+        kz = (occ >= 11.0) ? 1 : (int)(22.0 / (occ > 0.5 ? occ : 0.5) + 0.5);
+        if (kz < 2 && occ < 11.0) kz = 2;
+    }
+    if (kz > FC_KZ_MAX) kz = FC_KZ_MAX;
+    if (kz < 1 || g.n < 8) kz = 1;
+    const int nzu = (g.n + kz - 1) / kz;
+    const dim3 grid((nzu + FC_WARPS - 1) / FC_WARPS, g.n, g.n);
+    const double rl = s->rc + s->skin;
+    FcConst K;
+    memset(&K, 0, sizeof(K));
+    K.rc2_hi = (float)(rl * rl);                               // the filter's radius; nothing is evaluated
+    K.h = 0.5f * g.side;
+    K.hd = (double)K.h;
+    K.kz = kz;
+    K.nzu = nzu;
+    const double reach_xy = 1.5 * (double)g.last, reach_z = (0.5 * kz + 1.0) * (double)g.last;
+    K.thr_margin = (float)(2.0e-5 * (2.0 * reach_xy * reach_xy + reach_z * reach_z) + 1e-6 * rl * rl);
+    FcList LO;
+    LO.list = s->vl_list;
+    LO.count = s->vl_count;
+    LO.overflow = &s->vl_ctl->overflow;
+    LO.npad = s->vl_npad;
+    LO.cap = s->vl_cap;
+    k_force_cell_warp<false, true><<<grid, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, g, s->pp, K, s->frc, nullptr, nullptr, LO, cond);
+    CKL(s);
     return MD_OK;
 }

@@ -95,7 +95,8 @@ static void setup_grid(md_sim *s)
 {
     s->grid_paper_n = (int)floor(s->L / s->rc);
     make_grid(s, s->rc, s->grid);
-    make_grid(s, s->rc + s->skin, s->vgrid);         // neighbour-list path: cells of side >= rc + skin
+    make_grid(s, s->rc + s->skin + 1e-3, s->vgrid);  // neighbour-list path: cells wider than rc + skin (margin: see
+                                                     // the list mode of force_cell.cu)
 }
 
 static void setup_pair(md_sim *s)
@@ -588,6 +589,8 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
         if (R != 1 && R != 2 && R != 4 && R != 8) return MD_EINVAL;
         ljmd_ap_set_R(s, R);
         s->layout = LAYOUT_NONE;
+    } else if (!strcmp(key, "vl_naive_build")) {
+        s->vl_naive_build = value != 0.0;
     } else if (!strcmp(key, "skin")) {
         if (!(value > 0) || s->vl_list) return MD_EINVAL;          // before the first use of MD_VERLET
         s->skin = value;

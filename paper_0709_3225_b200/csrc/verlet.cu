@@ -21,6 +21,12 @@
 
 #define VL_T 128                      // threads per block of the list and force kernels
 #define VL_Q 10                       // queued FP64 pairs per thread
+#ifndef VL_U
+#define VL_U 4                        // list entries (gathers) in flight per thread
+#endif
+#ifndef VL_MINB
+#define VL_MINB 8
+#endif
 #define VL_JMASK 0x7fffffu
 
 // offset code of one dimension: 0: same cell, 1: +side, 2: -side, 3: +last, 4: -last
@@ -218,7 +224,7 @@ __device__ __forceinline__ void vl_precise(const float4 *__restrict__ lpos, cons
 }
 
 template <bool MODE2>
-__global__ void __launch_bounds__(VL_T, 8)
+__global__ void __launch_bounds__(VL_T, VL_MINB)
 k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams P, VlConst K,
            const unsigned *__restrict__ list, const int *__restrict__ count, float4 *__restrict__ frc,
            double *__restrict__ part_pe, double *__restrict__ part_w)
@@ -241,15 +247,15 @@ k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams 
         const unsigned *row = list + i;
         // four list entries per iteration: the coalesced list reads and the four gathers are all
         // issued before the first pair term (the kernel is bound by the latency of the gathers)
-        for (int k = 0; k < cnt; k += 4) {
-            unsigned e[4];
-            float4 lj[4];
+        for (int k = 0; k < cnt; k += VL_U) {
+            unsigned e[VL_U];
+            float4 lj[VL_U];
 #pragma unroll
-            for (int u = 0; u < 4; u++) e[u] = (k + u < cnt) ? row[(size_t)(k + u) * npad] : (unsigned)i;
+            for (int u = 0; u < VL_U; u++) e[u] = (k + u < cnt) ? row[(size_t)(k + u) * npad] : (unsigned)i;
 #pragma unroll
-            for (int u = 0; u < 4; u++) lj[u] = lpos[e[u] & VL_JMASK];
+            for (int u = 0; u < VL_U; u++) lj[u] = lpos[e[u] & VL_JMASK];
 #pragma unroll
-            for (int u = 0; u < 4; u++) {
+            for (int u = 0; u < VL_U; u++) {
                 const float4 o = offt[e[u] >> 23];
                 const float dx = (lj[u].x - li.x) + o.x, dy = (lj[u].y - li.y) + o.y, dz = (lj[u].z - li.z) + o.z;
                 float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
@@ -386,9 +392,11 @@ int ljmd_forces_verlet(md_sim *s)
     k_vl_copyback<<<nb, 256, 0, s->stream>>>(s->pos, s->vel, s->vl_lbuild, s->pos2, s->vel2, s->lpos, N, s->vl_ctl);
     CKL(s);
     const double rl = s->rc + s->skin;
-    k_vl_build<<<nbl, VL_T, 0, s->stream>>>(s->lpos, s->cell_start, N, s->vl_npad, g, (float)(rl * rl), s->vl_cap, s->vl_list,
-                                            s->vl_count, s->vl_ctl);
-    CKL(s);
+    if (s->vl_naive_build) {
+        k_vl_build<<<nbl, VL_T, 0, s->stream>>>(s->lpos, s->cell_start, N, s->vl_npad, g, (float)(rl * rl), s->vl_cap, s->vl_list,
+                                                s->vl_count, s->vl_ctl);
+        CKL(s);
+    } else if ((r = ljmd_vl_build_lists(s, &s->vl_ctl->rebuild))) return r;
     ljmd_tick(s, TAG_BUILD);
     if (nbl > s->part_cap) return MD_ENOMEM;
     double *ppe = s->part + (size_t)s->part_cap;
