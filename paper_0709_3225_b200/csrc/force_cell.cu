@@ -435,8 +435,16 @@ k_force_cell_warp(const float4 *__restrict__ lpos, const int *__restrict__ cell_
     if (LIST && cond && !*cond) return;                         // conditional launch (verlet.cu)
     __shared__ FcWarp sm[FC_WARPS];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int zu = blockIdx.x * FC_WARPS + wid;
-    const int n = g.n, cx = blockIdx.z, cy = blockIdx.y;
+    const int n = g.n;
+    // force mode: grid = (groups per column / FC_WARPS, n, n).  List mode: a small 1-D grid loops over the
+    // same block indices, so that the launch costs nothing on the steps that do not rebuild.
+    const int gx = (K.nzu + FC_WARPS - 1) / FC_WARPS;
+    const int nblk = LIST ? gx * n * n : 1;
+    for (int blk = LIST ? (int)blockIdx.x : 0; blk < nblk; blk += LIST ? (int)gridDim.x : 1) {
+    const int bx = LIST ? blk % gx : (int)blockIdx.x;
+    const int cy = LIST ? (blk / gx) % n : (int)blockIdx.y;
+    const int cx = LIST ? blk / (gx * n) : (int)blockIdx.z;
+    const int zu = bx * FC_WARPS + wid;
     double pe = 0.0, w = 0.0;
     if (zu < K.nzu) {
         const int z0 = zu * K.kz, kk = min(K.kz, n - z0);
@@ -512,13 +520,14 @@ k_force_cell_warp(const float4 *__restrict__ lpos, const int *__restrict__ cell_
             fc_cell<MODE2, LIST>(S, lpos, cell_start, G, P, K, frc, pe, w, LO);
         }
     }
-    if (LIST) return;
+    if (LIST) { __syncwarp(); continue; }
     pe = warp_sum(pe);
     w = warp_sum(w);
     if (lane == 0) {
-        const int u = (cx * n + cy) * (gridDim.x * FC_WARPS) + zu;
+        const int u = (cx * n + cy) * (gx * FC_WARPS) + zu;
         part_pe[u] = 0.5 * pe;                       // every pair is visited from both ends
         part_w[u] = 0.5 * w;
+    }
     }
 }
 
@@ -607,7 +616,9 @@ int ljmd_vl_build_lists(md_sim *s, const int *cond)
     LO.overflow = &s->vl_ctl->overflow;
     LO.npad = s->vl_npad;
     LO.cap = s->vl_cap;
-    k_force_cell_warp<false, true><<<grid, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, g, s->pp, K, s->frc, nullptr, nullptr, LO, cond);
+    int nblk = (int)(grid.x * grid.y * grid.z), nres = 4 * 148 * 2;           // a few resident waves of blocks
+    if (nblk > nres) nblk = nres;
+    k_force_cell_warp<false, true><<<nblk, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, g, s->pp, K, s->frc, nullptr, nullptr, LO, cond);
     CKL(s);
     return MD_OK;
 }

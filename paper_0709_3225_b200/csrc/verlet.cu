@@ -113,12 +113,12 @@ k_vl_bin(const float4 *__restrict__ pos, int N, Grid g, int *__restrict__ cell_o
          int *__restrict__ cell_count, const VlCtl *__restrict__ ctl)
 {
     if (!ctl->rebuild) return;
-    const int i = blockIdx.x * 256 + threadIdx.x;
-    if (i >= N) return;
-    const float4 p = pos[i];
-    const int c = (vl_cell_coord(p.x, g) * g.n + vl_cell_coord(p.y, g)) * g.n + vl_cell_coord(p.z, g);
-    cell_of[i] = c;
-    rank[i] = atomicAdd(&cell_count[c], 1);
+    for (int i = blockIdx.x * 256 + threadIdx.x; i < N; i += gridDim.x * 256) {      // small grid: cheap when idle
+        const float4 p = pos[i];
+        const int c = (vl_cell_coord(p.x, g) * g.n + vl_cell_coord(p.y, g)) * g.n + vl_cell_coord(p.z, g);
+        cell_of[i] = c;
+        rank[i] = atomicAdd(&cell_count[c], 1);
+    }
 }
 
 // Scatter into cell order (to the spare buffers), with the cell-local coordinates.
@@ -129,20 +129,20 @@ k_vl_scatter(const float4 *__restrict__ pos, const float4 *__restrict__ vel, int
              const VlCtl *__restrict__ ctl)
 {
     if (!ctl->rebuild) return;
-    const int i = blockIdx.x * 256 + threadIdx.x;
-    if (i >= N) return;
-    const int c = cell_of[i];
-    const int dst = cell_start[c] + rank[i];
-    const float4 p = pos[i];
-    const int cz = c % g.n, cy = (c / g.n) % g.n, cx = c / (g.n * g.n);
-    float4 l;
-    l.x = p.x - (float)cx * g.side;                    // exact
-    l.y = p.y - (float)cy * g.side;
-    l.z = p.z - (float)cz * g.side;
-    l.w = __int_as_float(c);
-    pos2[dst] = p;
-    vel2[dst] = vel[i];
-    lpos[dst] = l;
+    for (int i = blockIdx.x * 256 + threadIdx.x; i < N; i += gridDim.x * 256) {
+        const int c = cell_of[i];
+        const int dst = cell_start[c] + rank[i];
+        const float4 p = pos[i];
+        const int cz = c % g.n, cy = (c / g.n) % g.n, cx = c / (g.n * g.n);
+        float4 l;
+        l.x = p.x - (float)cx * g.side;                    // exact
+        l.y = p.y - (float)cy * g.side;
+        l.z = p.z - (float)cz * g.side;
+        l.w = __int_as_float(c);
+        pos2[dst] = p;
+        vel2[dst] = vel[i];
+        lpos[dst] = l;
+    }
 }
 
 // The host never swaps buffers on this path (it does not know whether a build happened): copy back.
@@ -152,11 +152,11 @@ k_vl_copyback(float4 *__restrict__ pos, float4 *__restrict__ vel, float4 *__rest
               const VlCtl *__restrict__ ctl)
 {
     if (!ctl->rebuild) return;
-    const int i = blockIdx.x * 256 + threadIdx.x;
-    if (i >= N) return;
-    pos[i] = pos2[i];
-    vel[i] = vel2[i];
-    lbuild[i] = lpos[i];
+    for (int i = blockIdx.x * 256 + threadIdx.x; i < N; i += gridDim.x * 256) {
+        pos[i] = pos2[i];
+        vel[i] = vel2[i];
+        lbuild[i] = lpos[i];
+    }
 }
 
 // Neighbour list of every atom from the 27 cells around its home cell: r < rc + skin in exact
@@ -371,7 +371,8 @@ int ljmd_forces_verlet(md_sim *s)
 {
     int r = vl_alloc(s);
     if (r) return r;
-    const int N = (int)s->N, nb = (N + 255) / 256, nbl = (N + VL_T - 1) / VL_T;
+    const int N = (int)s->N, nbl = (N + VL_T - 1) / VL_T;
+    const int nb = min((N + 255) / 256, 148 * 16);            // grid-stride kernels: idle launches stay cheap
     const Grid &g = s->vgrid;
     if (s->layout != LAYOUT_VERLET) {
         if ((r = vl_force_build(s))) return r;
