@@ -164,8 +164,11 @@ def time_md(b, torch, sysd, algo, steps, warmup, flush, buf):
             tot += e0.elapsed_time(e1)
         flushed_ms = tot / steps
     ke, pe, w = s.energies()
+    vl100 = None
+    if algo == 2:
+        vl100 = 100.0 * s.stat("vl_builds") / max(1.0, s.stat("vl_steps"))
     s.close()
-    return dict(steady_ms=steady_ms, flushed_ms=flushed_ms, launches_per_step=launches / steps,
+    return dict(vl_builds_per_100=vl100, steady_ms=steady_ms, flushed_ms=flushed_ms, launches_per_step=launches / steps,
                 t_force_kernel_ms=t_force, phases_ms=phases, energy=ke + pe)
 
 
@@ -357,6 +360,15 @@ def run_ours(args):
                              "roofline_streaming_kernels": stream_roofline(osys["N"], rr["phases_ms"], peaks)
                              if ocfg["algo"] == 1 else None,
                              "launches_per_step": rr["launches_per_step"]}
+            if ocfg["algo"] == 1:
+                # the same system through the neighbour-list path (algo = MD_VERLET):
+                # an extension beyond the named configs, reported beside them
+                rv = time_md(b, torch, osys, b.MD_VERLET, max(osteps, 100), 5, False, buf)
+                others[oname + "_verlet"] = {"N": osys["N"], "atom_steps_per_s": osys["N"] / (rv["steady_ms"] * 1e-3),
+                                             "ms_per_step": rv["steady_ms"], "phases_ms": rv["phases_ms"],
+                                             "force_kernel_ms": rv["t_force_kernel_ms"],
+                                             "launches_per_step": rv["launches_per_step"],
+                                             "list_builds_per_100_steps": rv.get("vl_builds_per_100")}
         others["c5_rand48"] = bench_rand48(b, torch, 5, peaks)
         line["others"] = others
     if world > 1:
