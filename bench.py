@@ -231,6 +231,16 @@ def stream_roofline(N, phases_ms, peaks):
             "traffic": None, "kernel": "kick/drift/histogram + scan + scatter", "bytes_per_atom": CELL_STREAM_BYTES_PER_ATOM}
 
 
+def verlet_roofline(N, rho, rc, skin, t_kernel_ms, peaks, n_sms):
+    """List evaluation kernel: one distance test (8 flop) per list entry, ~19 flop per in-range pair."""
+    entries = N * NBR_PER_ATOM(rho, rc + skin)
+    flops = entries * FLOP_PER_PAIR_TEST + N * NBR_PER_ATOM(rho, rc) * FLOP_PER_INRANGE
+    peak = n_sms * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    ach = flops / (t_kernel_ms * 1e-3) / 1e12
+    return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+            "kernel": "neighbour-list force", "list_entries_per_s": entries / (t_kernel_ms * 1e-3)}
+
+
 def bench_rand48(b, torch, steps, peaks):
     """Config 5: 65536 streams x 4096 draws and one stream of 2^28 draws, uint32 and double."""
     res = {}
@@ -295,6 +305,8 @@ def run_ours(args):
     cfg = wl.CONFIGS[name]
     sysd = wl.md_system(name, gpu_uniform_source(b))
     algo = cfg["algo"]
+    if args.algo == "verlet":
+        algo = b.MD_VERLET
     buf = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")
     steps, warmup = args.steps, max(3, args.warmup)
 
@@ -311,11 +323,13 @@ def run_ours(args):
     value = whole_job_value(N, world, ms)
     if algo == 0:
         roof = allpairs_roofline(N, cfg["rho"], wl.RC, r["t_force_kernel_ms"], peaks, n_sms)
+    elif algo == 2:
+        roof = verlet_roofline(N, cfg["rho"], wl.RC, 0.3, r["t_force_kernel_ms"], peaks, n_sms)
     else:
         with b.Sim(N, sysd["L"]) as tmp:
             ncell = int(tmp.stat("ncell"))
         roof = cell_roofline(N, cfg["rho"], wl.RC, ncell, r["t_force_kernel_ms"], peaks, n_sms)
-    roof["traffic"] = ncu_traffic(name)
+    roof["traffic"] = ncu_traffic(name if algo != 2 else name + "_verlet")
     stream_roof = stream_roofline(N, r["phases_ms"], peaks) if algo == 1 else None
     roof["kernel_ms"] = r["t_force_kernel_ms"]
     roof["kernel_share_of_step"] = r["phases_ms"]["force"] / max(1e-12, sum(r["phases_ms"].values()))
@@ -326,7 +340,7 @@ def run_ours(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "f32 state and distance filter, f64 in-range pair terms",
         "data": "synthetic",
         "config": {"workload": name, "N": N, "rho": cfg["rho"], "T": cfg["T"], "rc": wl.RC, "dt": wl.DT,
-                   "algo": "allpairs" if algo == 0 else "cell", "shifted": wl.SHIFTED,
+                   "algo": ("allpairs", "cell", "verlet")[algo], "shifted": wl.SHIFTED,
                    "l2": "flushed between steps (256 MB read-modify-write); steady_state is the unflushed md_step(K) loop",
                    "parallelism": "replicas x%d" % world if world > 1 else "single GPU"},
         "steady_state": {"ms_per_step": r["steady_ms"], "value": world * N / (r["steady_ms"] * 1e-3)},
@@ -341,7 +355,7 @@ def run_ours(args):
     }
     if rank == 0 and world == 1:
         nb = 2 if algo == 0 and N >= 20000 else (20 if N <= 4000 else 3)
-        cb = cpu_baseline_md(sysd, algo, nb)
+        cb = cpu_baseline_md(sysd, min(algo, 1), nb)           # the oracle has two loops: all-pairs and cell list
         line["cpu_baseline"] = {"value": cb["value"], "unit": "atom-steps/s", "cores": cb["cores"], "kind": "oracle",
                                 "sample": "%d force evaluations (%d velocity-Verlet steps) of the same N=%d system, %.1f s"
                                           % (cb["evals"], nb, N, cb["seconds"])}
@@ -422,6 +436,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c2_allpairs_32k", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--algo", default=None, choices=["verlet"],
+                    help="run the workload's system through the neighbour-list path instead of its named path")
     ap.add_argument("--no-others", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
