@@ -23,7 +23,9 @@
 
 #define FC_WARPS 4
 #define FC_T (FC_WARPS * 32)
+#ifndef FC_CAP
 #define FC_CAP 544                    // staged candidates per pass (27 list cells of 18.5 atoms fit)
+#endif
 #define FC_STEPS (FC_CAP / 32)
 #define FC_CLOSE 8                    // queued FP64 pairs per lane
 #ifndef FC_KZ_MAX
