@@ -145,3 +145,22 @@ def test_full_size_parity(b, name, steps):
     for a, c in bad:
         assert abs(F[a, c] - Fo[a, c]) < 0.04 + 1e-4
     assert pe == pytest.approx(peo, rel=1e-6) and w == pytest.approx(wo, rel=1e-6)
+
+
+@pytest.mark.parametrize("n,rho", [(8, 0.8), (10, 0.3), (9, 0.05)])
+def test_both_list_builders_give_the_same_lists(b, n, rho):
+    """Lists written by the cell kernel's filter (default) and by the plain thread-per-atom kernel
+    ("vl_naive_build"): same forces to rounding, same energies, both within R15 of the oracle."""
+    pos, L = wl.perturbed_fcc(n, rho, 0.12, seed=40 + n)
+    Fo, peo, wo = oracle.forces(pos.astype(np.float64), L, algo=0)
+    res = []
+    for naive in (0, 1):
+        with b.Sim(pos.shape[0], L) as s:
+            s.option("vl_naive_build", naive)
+            s.set_state(pos, np.zeros_like(pos))
+            s.compute_forces(b.MD_VERLET)
+            res.append((s.forces(), s.energies()))
+            assert force_check(res[-1][0], Fo)[0] == 0
+    # the two kernels write the entries in different orders: FP32 sums agree to rounding
+    assert np.all(np.abs(res[0][0] - res[1][0]) <= 1e-5 + 2e-6 * np.abs(res[1][0]))
+    assert res[0][1][1] == pytest.approx(res[1][1][1], rel=1e-7) and res[0][1][1] == pytest.approx(peo, rel=1e-6)
