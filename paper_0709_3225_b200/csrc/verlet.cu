@@ -28,6 +28,7 @@
 #define VL_MINB 8
 #endif
 #define VL_JMASK 0x7fffffu
+#define VL_INERT (31u << 23)            // offset index 31 = (+side, +side, +side): beyond any cutoff
 
 // offset code of one dimension: 0: same cell, 1: +side, 2: -side, 3: +last, 4: -last
 __device__ __forceinline__ float vl_code_value(int code, const Grid &g)
@@ -202,8 +203,11 @@ k_vl_build(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, 
             }
         }
     }
-    count[i] = min(cnt, cap);
     if (cnt > cap) ctl->overflow = 1;
+    cnt = min(cnt, cap);
+    // pad to a multiple of VL_U with inert entries: the atom itself, displaced by a cell diagonal
+    for (; cnt % VL_U; cnt++) list[(size_t)cnt * npad + i] = (unsigned)i | VL_INERT;
+    count[i] = cnt;
 }
 
 struct VlConst {
@@ -247,19 +251,20 @@ k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams 
         const unsigned *row = list + i;
         // four list entries per iteration: the coalesced list reads and the four gathers are all
         // issued before the first pair term (the kernel is bound by the latency of the gathers)
-        for (int k = 0; k < cnt; k += VL_U) {
+        // (the builders pad every list to a multiple of VL_U entries with inert ones: no validity tests here)
+        const size_t stride = (size_t)npad;
+        for (int k = 0; k < cnt; k += VL_U, row += VL_U * stride) {
             unsigned e[VL_U];
             float4 lj[VL_U];
 #pragma unroll
-            for (int u = 0; u < VL_U; u++) e[u] = (k + u < cnt) ? row[(size_t)(k + u) * npad] : (unsigned)i;
+            for (int u = 0; u < VL_U; u++) e[u] = row[u * stride];
 #pragma unroll
             for (int u = 0; u < VL_U; u++) lj[u] = lpos[e[u] & VL_JMASK];
 #pragma unroll
             for (int u = 0; u < VL_U; u++) {
                 const float4 o = offt[e[u] >> 23];
                 const float dx = (lj[u].x - li.x) + o.x, dy = (lj[u].y - li.y) + o.y, dz = (lj[u].z - li.z) + o.z;
-                float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                r2 = (k + u < cnt) ? r2 : 3.0e38f;                      // padding slot: contributes nothing
+                const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
                 // p2 <= r2 < rc2_lo: FP32 term; the steep part and the sliver around rc^2: FP64 (queued)
                 const bool fast = r2 >= K.p2 && r2 < K.rc2_lo;
                 if (!fast && r2 < K.rc2_hi) {
@@ -291,6 +296,7 @@ k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams 
         if (nq <= VL_Q) {
             for (int q = 0; q < nq; q++) vl_precise(lpos, offt, P, li, queue[q][threadIdx.x], dfx, dfy, dfz, dpe, dw);
         } else {
+            row = list + i;
             for (int k = 0; k < cnt; k++) {
                 const unsigned e = row[(size_t)k * npad];
                 const float4 lj = lpos[e & VL_JMASK];
@@ -326,7 +332,7 @@ static int vl_alloc(md_sim *s)
     const double rl = s->rc + s->skin;
     const double mean = 4.0 / 3.0 * 3.14159265358979 * rl * rl * rl * (double)s->N / (s->L * s->L * s->L);
     int cap = (int)(1.4 * mean) + 32;
-    cap = (cap + 7) / 8 * 8;
+    cap = (cap + 7) / 8 * 8;                                            // a multiple of VL_U: padding always fits
     s->vl_cap = cap;
     s->vl_npad = (int)((s->N + 31) / 32 * 32);
     s->vl_list = (unsigned *)ljmd_dev_alloc((size_t)cap * s->vl_npad * sizeof(unsigned), s->stream);
