@@ -350,6 +350,18 @@ extern "C" int md_get_state(md_sim *s, float *pos, float *vel)
     if (!s) return MD_EINVAL;
     if (!s->has_state) return MD_ESTATE;
     int r;
+    if (pos && vel) {
+        // both arrays with one synchronisation: positions through xfer, velocities through the spare
+        // scatter target pos2 (dead between force evaluations)
+        float *stage2 = (float *)s->pos2;
+        if ((r = ljmd_unpack(s, s->pos, s->xfer))) return r;
+        if ((r = ljmd_unpack(s, s->vel, stage2))) return r;
+        const size_t bytes = (size_t)s->N * 3 * sizeof(float);
+        CK(cudaMemcpyAsync(pos, s->xfer, bytes, cudaMemcpyDefault, s->stream));
+        CK(cudaMemcpyAsync(vel, stage2, bytes, cudaMemcpyDefault, s->stream));
+        CK(cudaStreamSynchronize(s->stream));
+        return MD_OK;
+    }
     if (pos && (r = read_out(s, s->pos, pos))) return r;
     if (vel && (r = read_out(s, s->vel, vel))) return r;
     return MD_OK;
