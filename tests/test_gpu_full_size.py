@@ -104,7 +104,8 @@ def test_c4_cell_2048000(b, name):
 
 
 @pytest.mark.parametrize("name,algo,nsteps", [("c1_allpairs_500", 0, 10000), ("c1_allpairs_500", 1, 10000),
-                                              ("c3_cell_256k", 1, 10000)])
+                                              ("c3_cell_256k", 1, 10000), ("c1_allpairs_500", 2, 10000),
+                                              ("c3_cell_256k", 2, 10000)])
 def test_nve_drift_10k_steps(b, name, algo, nsteps):
     """R17: |<E>_{9000..10000} - <E>_{1000..2000}| / |E(0)| < 1e-4, E sampled every 10 steps."""
     sysd = wl.md_system(name, gpu_uniforms(b))
