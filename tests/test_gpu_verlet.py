@@ -164,3 +164,21 @@ def test_both_list_builders_give_the_same_lists(b, n, rho):
     # the two kernels write the entries in different orders: FP32 sums agree to rounding
     assert np.all(np.abs(res[0][0] - res[1][0]) <= 1e-5 + 2e-6 * np.abs(res[1][0]))
     assert res[0][1][1] == pytest.approx(res[1][1][1], rel=1e-7) and res[0][1][1] == pytest.approx(peo, rel=1e-6)
+
+
+def test_eps_sigma_not_one(b):
+    """Scaled units (R1): sigma = 1.7, eps = 0.4, rc = 2.5 sigma; skin defaults to 0.3 sigma."""
+    sigma, eps = 1.7, 0.4
+    pos, L = wl.perturbed_fcc(6, 0.8, 0.1, seed=21)
+    pos = (pos.astype(np.float64) * sigma).astype(np.float32)
+    L = float(np.float32(L * sigma))
+    Fo, peo, wo = oracle.forces(pos.astype(np.float64), L, rc=2.5 * sigma, eps=eps, sigma=sigma, algo=0)
+    with b.Sim(pos.shape[0], L, rc=2.5 * sigma, eps=eps, sigma=sigma) as s:
+        s.set_state(pos, np.zeros_like(pos))
+        s.compute_forces(b.MD_VERLET)
+        F = s.forces().astype(np.float64)
+        ke, pe, w = s.energies()
+    # the tolerance of R15 is stated in units of eps / sigma
+    tol = np.maximum(1e-4 * np.abs(Fo), 1e-5 * eps / sigma)
+    assert np.all(np.abs(F - Fo) <= tol)
+    assert pe == pytest.approx(peo, rel=1e-6) and w == pytest.approx(wo, rel=1e-6)
