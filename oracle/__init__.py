@@ -66,6 +66,8 @@ def lib():
         L.rand48_skip.restype = u64
         L.rand48_leapfrog.argtypes = [u64, i64, i64, vp]
         L.rand48_leapfrog.restype = None
+        L.mb_velocities.argtypes = [i64, d, ctypes.POINTER(u64), vp]
+        L.mb_velocities.restype = None
         _lib = L
     return _lib
 
@@ -176,3 +178,12 @@ def rand48_leapfrog(seed, S, ndraws):
     out = np.zeros(ndraws, dtype=np.uint64)
     lib().rand48_leapfrog(seed, S, ndraws, _ptr(out))
     return out
+
+
+def mb_velocities(N, T, seed48):
+    """Maxwell-Boltzmann velocities [N,3] (FP64) from one rand48 stream started at state seed48, zero
+    net momentum, sum v^2 = 3 N T; also returns the state after the 6 N draws.  SURVEY 8(d) recipe."""
+    vel = np.zeros((N, 3), dtype=np.float64)
+    st = ctypes.c_uint64(int(seed48))
+    lib().mb_velocities(N, float(T), ctypes.byref(st), _ptr(vel))
+    return vel, st.value

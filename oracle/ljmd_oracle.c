@@ -396,3 +396,39 @@ void rand48_leapfrog(uint64_t seed, int64_t S, int64_t ndraws, uint64_t *out)
         }
     free(lane);
 }
+
+/* ------------------------------------------------------------------ O6 --
+ * Maxwell-Boltzmann start velocities from ONE rand48 stream (SURVEY 8(d) input recipe, DESIGN.md
+ * section 4; the paper names rand48 as the generator for such uses).
+ * For atom i, component c, in order: u1, u2 = the next two draws x * 2^-48;
+ *     v = sqrt(T) sqrt(-2 ln(1 - u1)) cos(2 pi u2);
+ * then the mean over the atoms is subtracted per component and all velocities are scaled so
+ * that sum v^2 = 3 N T (R11).  vel: [N][3] doubles out; *state: in the start state x0, out the
+ * state after the 6 N draws.  The GPU counterpart is md_init_velocities.
+ */
+void mb_velocities(int64_t N, double T, uint64_t *state, double *vel)
+{
+    const double two_pi = 6.283185307179586476925286766559;
+    uint64_t x = *state;
+    double mean[3] = {0.0, 0.0, 0.0};
+    for (int64_t i = 0; i < N; i++)
+        for (int c = 0; c < 3; c++) {
+            x = rand48_next(x);
+            double u1 = (double)x * 0x1p-48;
+            x = rand48_next(x);
+            double u2 = (double)x * 0x1p-48;
+            double v = sqrt(T) * sqrt(-2.0 * log(1.0 - u1)) * cos(two_pi * u2);
+            vel[3 * i + c] = v;
+            mean[c] += v;
+        }
+    for (int c = 0; c < 3; c++) mean[c] /= (double)N;
+    double s2 = 0.0;
+    for (int64_t i = 0; i < N; i++)
+        for (int c = 0; c < 3; c++) {
+            vel[3 * i + c] -= mean[c];
+            s2 += vel[3 * i + c] * vel[3 * i + c];
+        }
+    double scale = sqrt(3.0 * (double)N * T / s2);
+    for (int64_t k = 0; k < 3 * N; k++) vel[k] *= scale;
+    *state = x;
+}

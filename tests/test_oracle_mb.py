@@ -1,0 +1,43 @@
+"""Pins of the oracle's Maxwell-Boltzmann generator (oracle.mb_velocities): the printed values of the
+survey's independent NumPy probe (tests/golden/config1_trajectory.txt), the harness generator
+(workloads.maxwell_boltzmann fed with the oracle's sequential rand48), and the defining moments."""
+import numpy as np
+import pytest
+
+import oracle
+from conftest import golden_lines
+from paper_0709_3225_b200 import workloads as wl
+
+
+@pytest.fixture(scope="module")
+def g():
+    return {row[0]: row[1:] for row in golden_lines("config1_trajectory.txt")}
+
+
+def test_config1_values_of_the_survey_probe(g):
+    x0 = wl.splitmix64(wl.MASTER_SEED) & wl.MASK48
+    assert x0 == int(g["rand48_start_state"][0], 16)
+    v, x1 = oracle.mb_velocities(500, 1.0, x0)
+    assert x1 == int(g["rand48_state_after_3000_draws"][0], 16)          # exactly 6 N draws, in order
+    # the probe printed the FP32 state to 8 decimals
+    assert v[0].astype(np.float32).astype(np.float64) == pytest.approx([float(t) for t in g["vel0"]], abs=1e-8)
+    v32 = v.astype(np.float32).astype(np.float64)
+    assert 0.5 * np.sum(v32 * v32) == pytest.approx(float(g["step0"][1]), rel=1e-9)   # KE of the FP32 state
+
+
+@pytest.mark.parametrize("N,T,seed", [(500, 1.0, 1), (4000, 1.2, 77), (7, 0.3, 12345)])
+def test_matches_the_harness_generator_and_the_moments(N, T, seed, oracle_uniforms):
+    x0 = wl.splitmix64(seed) & wl.MASK48
+    v, _ = oracle.mb_velocities(N, T, x0)
+    ref = wl.maxwell_boltzmann(oracle_uniforms(x0, 6 * N), N, T)        # float32
+    assert np.max(np.abs(v - ref.astype(np.float64))) < 3e-7             # FP32 cast of the same numbers
+    assert np.max(np.abs(v.sum(axis=0))) < 1e-10 * N                      # zero net momentum
+    assert np.sum(v * v) == pytest.approx(3.0 * N * T, rel=1e-13)         # R11
+
+
+def test_draw_order_is_atom_major_component_minor():
+    """u1 of (atom 0, x) is the first draw: a state chosen so that 1 - u1 = 1 gives v_x = 0 before the
+    mean is removed; checked through the second atom instead: velocities of a 2-atom system are
+    antisymmetric after the mean is removed."""
+    v, _ = oracle.mb_velocities(2, 1.0, 0x1234ABCD330E)
+    assert np.allclose(v[0], -v[1], rtol=0, atol=1e-14)
