@@ -80,6 +80,14 @@ int md_compute_forces(md_sim *s, int algo);
  * coincident atoms are undefined behaviour. */
 int md_step(md_sim *s, int64_t nsteps, int algo);
 
+/* Maxwell-Boltzmann start velocities on the device (an extension: SURVEY 8(f) item 3; the paper names
+ * rand48 as the generator for such uses).  One rand48 stream started at state
+ * seed48 (< 2^48); atom i (caller's order) consumes draws 6 i .. 6 i + 5: per component u1, u2 and
+ * v = sqrt(T) sqrt(-2 ln(1 - u1)) cos(2 pi u2); then the mean is removed and the set rescaled so that
+ * sum v^2 = 3 N T; stored as FP32.  Needs md_set_state first (MD_ESTATE); positions and forces are
+ * untouched, KE is refreshed.  MD_EINVAL: T <= 0, seed48 >= 2^48, N < 2. */
+int md_init_velocities(md_sim *s, double T, uint64_t seed48);
+
 /* Forces [N][3] at the current positions, caller's atom order.  MD_ESTATE if stale. */
 int md_get_forces(md_sim *s, float *f);
 

@@ -40,6 +40,7 @@ _SIGS = {
     "md_get_energies": ([_vp, _pd, _pd, _pd], _i32),
     "rand48_fill": ([_vp, _i64, _i64, _i32, _vp], _i32),
     "md_strerror": ([_i32], ctypes.c_char_p),
+    "md_init_velocities": ([_vp, ctypes.c_double, ctypes.c_uint64], _i32),
     "md_set_stream": ([_vp, _vp], _i32),
     "rand48_set_stream": ([_vp], _i32),
     "md_set_allocator": ([ALLOC_FN, FREE_FN], _i32),
@@ -133,6 +134,10 @@ def rand48_fill(seeds, nstreams, ndraws, kind, out):
     _check(_lib.rand48_fill(_addr(seeds), nstreams, ndraws, kind, _addr(out)), "rand48_fill")
 
 
+def md_init_velocities(h, T, seed48):
+    _check(_lib.md_init_velocities(h, float(T), int(seed48)), "md_init_velocities")
+
+
 def md_set_stream(h, stream):
     _check(_lib.md_set_stream(h, stream), "md_set_stream")
 
@@ -201,6 +206,9 @@ class Sim:
         vel = np.ascontiguousarray(vel, dtype=np.float32)
         assert pos.shape == (self.N, 3) and vel.shape == (self.N, 3)
         md_set_state(self.h, pos, vel)
+
+    def init_velocities(self, T, seed48):
+        md_init_velocities(self.h, T, seed48)
 
     def get_state(self):
         pos = np.empty((self.N, 3), dtype=np.float32)

@@ -162,6 +162,7 @@ int ljmd_forces_allpairs(md_sim *s);
 void ljmd_ap_plan(md_sim *s);
 void ljmd_ap_set_R(md_sim *s, int R);                       // R in {0 (general kernel), 1, 2, 4, 8}
 int ljmd_scan_counts(md_sim *s, int *count, int *start, int n, const int *cond = nullptr);   // exclusive scan, zeroes count; cond: device flag, 0 = do nothing
+int ljmd_mb_velocities(md_sim *s, double T, uint64_t seed48, double *vraw, double *part, double *mom);   // rand48.cu
 int ljmd_vl_kick_drift(md_sim *s, int kicks);
 int ljmd_vl_build_lists(md_sim *s, const int *cond);    // force_cell.cu: lists through the cell kernel's filter
 int ljmd_forces_verlet(md_sim *s);

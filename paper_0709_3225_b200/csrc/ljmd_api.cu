@@ -367,6 +367,27 @@ extern "C" int md_get_state(md_sim *s, float *pos, float *vel)
     return MD_OK;
 }
 
+extern "C" int md_init_velocities(md_sim *s, double T, uint64_t seed48)
+{
+    if (!s || !(T > 0) || !isfinite(T) || (seed48 >> 48)) return MD_EINVAL;
+    if (!s->has_state) return MD_ESTATE;                              // positions (and atom ids) first
+    if (s->N < 2) return MD_EINVAL;                                   // the rescaling needs a spread
+    const int nb = (int)((s->N + 255) / 256);
+    const int64_t nscratch = 3 * s->N + 4 * (int64_t)nb + 4;
+    double *scratch = (double *)ljmd_dev_alloc(nscratch * (int64_t)sizeof(double), s->stream);
+    if (!scratch) return MD_ENOMEM;
+    int r = ljmd_mb_velocities(s, T, seed48, scratch, scratch + 3 * s->N, scratch + 3 * s->N + 4 * (int64_t)nb);
+    if (r == MD_OK && s->forces_valid) {                              // forces do not depend on v; KE does
+        r = ljmd_ke_only(s);
+        if (r == MD_OK) r = ljmd_reduce_energies(s);
+    }
+    cudaError_t e = cudaStreamSynchronize(s->stream);
+    ljmd_dev_free(scratch, s->stream);
+    if (r) return r;
+    if (e != cudaSuccess) { ljmd_note_cuda_error(e, "md_init_velocities", __FILE__, __LINE__); return MD_ECUDA; }
+    return MD_OK;
+}
+
 extern "C" int md_get_forces(md_sim *s, float *f)
 {
     if (!s || !f) return MD_EINVAL;

@@ -238,3 +238,91 @@ done:
     if (!out_dev && dout && dout != out) { cudaStreamSynchronize(st); ljmd_dev_free(dout, st); }
     return rc;
 }
+
+// ---------------------------------------------------------------------------------------
+// Maxwell-Boltzmann start velocities on the device (first half): the rand48 draws
+// are consumed in registers instead of being stored to HBM (PAPER.md:176-178 names that store as the
+// cost of the generator).  Atom `id` owns draws 6 id .. 6 id + 5 of ONE stream and reaches them by
+// skip-ahead; per component u1, u2 -> v = sqrt(T) sqrt(-2 ln(1 - u1)) cos(2 pi u2) in FP64; then the
+// mean is removed and the set rescaled to sum v^2 = 3 N T (R11).  Same recipe as oracle mb_velocities.
+#define MB_T 256
+
+__global__ void __launch_bounds__(MB_T)
+k_mb_draw(const float4 *__restrict__ pos, int64_t N, uint64_t x0, double sqrtT, double *__restrict__ vraw,
+          double *__restrict__ part)                                    // part: [4][gridDim.x] sums of vx, vy, vz, v^2
+{
+    __shared__ double red[32];
+    const int64_t slot = (int64_t)blockIdx.x * MB_T + threadIdx.x;
+    double v[3] = {0.0, 0.0, 0.0};
+    if (slot < N) {
+        const uint64_t id = (uint64_t)__float_as_int(pos[slot].w);         // caller's atom index
+        uint64_t x = r48_skip(x0, 6ull * id);
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            x = (R48_A * x + R48_C) & R48_MASK;
+            const double u1 = R48Out<2>::cv(x);
+            x = (R48_A * x + R48_C) & R48_MASK;
+            const double u2 = R48Out<2>::cv(x);
+            v[c] = sqrtT * sqrt(-2.0 * log(1.0 - u1)) * cos(6.283185307179586476925286766559 * u2);
+            vraw[3 * slot + c] = v[c];
+        }
+    }
+    const double q[4] = {v[0], v[1], v[2], v[0] * v[0] + v[1] * v[1] + v[2] * v[2]};
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        const double t = block_sum(q[k], red);
+        if (threadIdx.x == 0) part[(size_t)k * gridDim.x + blockIdx.x] = t;
+    }
+}
+
+// mean[3] and scale from the block partials: sum (v - m)^2 = sum v^2 - N m^2.  One block.
+__global__ void __launch_bounds__(1024)
+k_mb_moments(const double *__restrict__ part, int nblocks, int64_t N, double T, double *__restrict__ mom)
+{
+    __shared__ double red[32];
+    __shared__ double tot[4];
+    for (int k = 0; k < 4; k++) {
+        double a = 0.0;
+        for (int i = threadIdx.x; i < nblocks; i += blockDim.x) a += part[(size_t)k * nblocks + i];
+        a = block_sum(a, red);
+        if (threadIdx.x == 0) tot[k] = a;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const double n = (double)N;
+        const double mx = tot[0] / n, my = tot[1] / n, mz = tot[2] / n;
+        const double s2 = tot[3] - n * (mx * mx + my * my + mz * mz);
+        mom[0] = mx; mom[1] = my; mom[2] = mz;
+        mom[3] = sqrt(3.0 * n * T / s2);
+    }
+}
+
+__global__ void __launch_bounds__(MB_T)
+k_mb_apply(float4 *__restrict__ vel, const double *__restrict__ vraw, const double *__restrict__ mom, int64_t N)
+{
+    const int64_t slot = (int64_t)blockIdx.x * MB_T + threadIdx.x;
+    if (slot >= N) return;
+    const double sc = mom[3];
+    vel[slot] = make_float4((float)((vraw[3 * slot] - mom[0]) * sc), (float)((vraw[3 * slot + 1] - mom[1]) * sc),
+                            (float)((vraw[3 * slot + 2] - mom[2]) * sc), 0.f);
+}
+
+// vraw: [3 N] doubles, part: [4 * nblocks] doubles, mom: [4] doubles (device scratch of the caller)
+int ljmd_mb_velocities(md_sim *s, double T, uint64_t seed48, double *vraw, double *part, double *mom)
+{
+    cudaStream_t st = s->stream;
+    if (!g_r48_table_ready) {
+        k_r48_init_table<<<1, 1, 0, st>>>();
+        CK(cudaGetLastError());
+        g_r48_launches++;
+        g_r48_table_ready = true;
+    }
+    const int nb = (int)((s->N + MB_T - 1) / MB_T);
+    k_mb_draw<<<nb, MB_T, 0, st>>>(s->pos, s->N, seed48, sqrt(T), vraw, part);
+    CKL(s);
+    k_mb_moments<<<1, 1024, 0, st>>>(part, nb, s->N, T, mom);
+    CKL(s);
+    k_mb_apply<<<nb, MB_T, 0, st>>>(s->vel, vraw, mom, s->N);
+    CKL(s);
+    return MD_OK;
+}
