@@ -68,6 +68,8 @@ def lib():
         L.rand48_leapfrog.restype = None
         L.mb_velocities.argtypes = [i64, d, ctypes.POINTER(u64), vp]
         L.mb_velocities.restype = None
+        L.andersen_collide.argtypes = [i64, vp, d, ctypes.c_uint32, u64, i64]
+        L.andersen_collide.restype = i64
         _lib = L
     return _lib
 
@@ -187,3 +189,22 @@ def mb_velocities(N, T, seed48):
     st = ctypes.c_uint64(int(seed48))
     lib().mb_velocities(N, float(T), ctypes.byref(st), _ptr(vel))
     return vel, st.value
+
+
+def andersen_collide(vel, T, thr, seed48, t):
+    """Andersen thermostat collisions of step t on velocities vel [N,3] (FP64, copied): returns
+    (new velocities, number of collisions).  thr / 2^32 is the collision probability per atom and step."""
+    vel = _f64(vel).copy()
+    n = lib().andersen_collide(vel.shape[0], _ptr(vel), float(T), int(thr), int(seed48), int(t))
+    return vel, n
+
+
+def verlet_step(pos, vel, F, L, rc=2.5, eps=1.0, sigma=1.0, dt=0.005, mode=1, algo=0):
+    """One velocity-Verlet step in place on copies; returns pos, vel, F, (KE, PE, W).  PAPER.md:64."""
+    pos, vel, F = _f64(pos).copy(), _f64(vel).copy(), _f64(F).copy()
+    ke, pe, w = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    rcode = lib().verlet_step(pos.shape[0], _ptr(pos), _ptr(vel), _ptr(F), L, rc, eps, sigma, dt, mode, algo,
+                              ctypes.byref(ke), ctypes.byref(pe), ctypes.byref(w))
+    if rcode != 0:
+        raise ValueError("verlet_step failed (cell list needs >= 3 cells per dimension)")
+    return pos, vel, F, (ke.value, pe.value, w.value)

@@ -432,3 +432,35 @@ void mb_velocities(int64_t N, double T, uint64_t *state, double *vel)
     for (int64_t k = 0; k < 3 * N; k++) vel[k] *= scale;
     *state = x;
 }
+
+/* ----------------------------------------------------------------- O6b --
+ * Andersen thermostat with rand48 (the paper names thermostats among the uses of
+ * its generator; the scheme itself is the textbook one of the paper's
+ * ref. [19]).  Reading taken (R24): after the second half-kick of step t (t = 0, 1, ... since
+ * the thermostat was switched on) every atom i collides independently with probability
+ * thr / 2^32: ONE rand48 stream with start state seed48; (t, i) owns the 7 draws starting at index
+ * 7 (t N + i).  Draw 0 decides: collision iff its 32 high bits (x >> 16) are < thr (an integer
+ * comparison, so both sides take the same decision).  Draws 1..6 give u1, u2 per component and
+ * v_c = sqrt(T) sqrt(-2 ln(1 - u1)) cos(2 pi u2); they are skipped when there is no collision.
+ * vel: [N][3] doubles, updated in place.  Returns the number of collisions.
+ */
+int64_t andersen_collide(int64_t N, double *vel, double T, uint32_t thr, uint64_t seed48, int64_t t)
+{
+    const double two_pi = 6.283185307179586476925286766559;
+    int64_t ncoll = 0;
+    uint64_t x = seed48;
+    /* sequential walk to the first draw of step t: plain and slow on purpose */
+    for (int64_t k = 0; k < 7 * t * N; k++) x = rand48_next(x);
+    for (int64_t i = 0; i < N; i++) {
+        uint64_t d[7];
+        for (int k = 0; k < 7; k++) { x = rand48_next(x); d[k] = x; }
+        if ((uint32_t)(d[0] >> 16) < thr) {
+            ncoll++;
+            for (int c = 0; c < 3; c++) {
+                double u1 = (double)d[1 + 2 * c] * 0x1p-48, u2 = (double)d[2 + 2 * c] * 0x1p-48;
+                vel[3 * i + c] = sqrt(T) * sqrt(-2.0 * log(1.0 - u1)) * cos(two_pi * u2);
+            }
+        }
+    }
+    return ncoll;
+}
