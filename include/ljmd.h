@@ -127,6 +127,16 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
  *                    the last) are replayed from a CUDA graph that holds one unit of steps (2 on the
  *                    cell path, 2 * sort_every on the sorted all-pairs path: the number of steps
  *                    after which the buffer roles repeat); 0 = launch every kernel directly
+ *   "andersen_nu", "andersen_T", "andersen_seed"
+ *                    Andersen thermostat (an extension: SURVEY 8(f) item 3; thermostats are among the uses
+ *                    the paper names for its generator): after the second
+ *                    half-kick of every step each atom takes, with probability nu * dt (as the 32-bit
+ *                    threshold floor(nu dt 2^32), md_get_stat "andersen_threshold"), a fresh velocity
+ *                    sqrt(T) sqrt(-2 ln(1 - u1)) cos(2 pi u2) per component.  One rand48 stream from state
+ *                    "andersen_seed" (< 2^48); step t since the last change of these options and atom i
+ *                    own draws 7 (t N + i) .. + 6 (the first decides, by integer comparison of its 32
+ *                    high bits).  Active once nu > 0 and T > 0; nu = 0 switches it off.  Steps are then
+ *                    launched directly (no graph, no folded half-kick).
  *   "skin"           MD_VERLET: list radius minus rc (default 0.3 sigma); only before the first use
  *   "cell_group"     cells of one z-column handled by one warp of the cell-force kernel (1..5);
  *                    0 (default) = chosen from the mean occupancy

@@ -127,6 +127,10 @@ struct md_sim {
     int forces_algo;
     bool use_graph;
     int sort_every;
+    // Andersen thermostat (options "andersen_nu", "andersen_T", "andersen_seed"); and_thr = 0: off
+    uint32_t and_thr;
+    double and_T, and_nu;
+    uint64_t and_seed, and_t;     // stream start state, steps since it was (re)configured
     bool precise_r2_user;         // "precise_r2" was set through md_set_option
     int cell_group;               // cells per row group of the cell-force kernel; 0 = automatic
     int64_t launches, steps_done;
@@ -162,6 +166,7 @@ int ljmd_forces_allpairs(md_sim *s);
 void ljmd_ap_plan(md_sim *s);
 void ljmd_ap_set_R(md_sim *s, int R);                       // R in {0 (general kernel), 1, 2, 4, 8}
 int ljmd_scan_counts(md_sim *s, int *count, int *start, int n, const int *cond = nullptr);   // exclusive scan, zeroes count; cond: device flag, 0 = do nothing
+int ljmd_kick_andersen(md_sim *s);                   // rand48.cu: second half-kick + thermostat + KE
 int ljmd_mb_velocities(md_sim *s, double T, uint64_t seed48, double *vraw, double *part, double *mom);   // rand48.cu
 int ljmd_vl_kick_drift(md_sim *s, int kicks);
 int ljmd_vl_build_lists(md_sim *s, const int *cond);    // force_cell.cu: lists through the cell kernel's filter

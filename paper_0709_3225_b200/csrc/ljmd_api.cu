@@ -574,6 +574,15 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
     // Interior steps (all but the first and the last) are identical launch sequences and are
     // replayed from a CUDA graph, one unit of steps per replay.
     int64_t k = 0;
+    if (s->and_thr) {
+        // Andersen thermostat: the collisions follow every second half-kick, so nothing is folded into
+        // the next step and the step index is a kernel argument (direct launches, no graph)
+        for (; k < nsteps; k++) {
+            if ((r = one_step(s, algo, 1, false))) return r;
+            if ((r = ljmd_kick_andersen(s))) return r;
+            ljmd_tick(s, TAG_INTEGRATE);
+        }
+    }
     while (k < nsteps) {
         if (k > 0 && k < nsteps - 1 && s->use_graph && !s->time_kernels) {
             const int unit = graph_unit(s, algo);
@@ -622,6 +631,24 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
         if (R != 1 && R != 2 && R != 4 && R != 8) return MD_EINVAL;
         ljmd_ap_set_R(s, R);
         s->layout = LAYOUT_NONE;
+    } else if (!strcmp(key, "andersen_nu") || !strcmp(key, "andersen_T") || !strcmp(key, "andersen_seed")) {
+        if (!strcmp(key, "andersen_nu")) {
+            if (!(value >= 0) || !isfinite(value)) return MD_EINVAL;
+            s->and_nu = value;
+        } else if (!strcmp(key, "andersen_T")) {
+            if (!(value > 0) || !isfinite(value)) return MD_EINVAL;
+            s->and_T = value;
+        } else {
+            if (!(value >= 0) || value >= 281474976710656.0 || value != floor(value)) return MD_EINVAL;
+            s->and_seed = (uint64_t)value;
+        }
+        // collision probability per atom and step nu dt as a 32-bit threshold; needs a temperature
+        double p = s->and_nu * s->dt;
+        if (p > 1.0) p = 1.0;
+        double thr = floor(p * 4294967296.0);
+        if (thr > 4294967295.0) thr = 4294967295.0;
+        s->and_thr = (s->and_T > 0) ? (uint32_t)thr : 0u;
+        s->and_t = 0;                                                 // the stream starts over
     } else if (!strcmp(key, "vl_naive_build")) {
         s->vl_naive_build = value != 0.0;
     } else if (!strcmp(key, "skin")) {
@@ -648,6 +675,8 @@ extern "C" int md_get_stat(md_sim *s, const char *key, double *value)
     else if (!strcmp(key, "kernel_launches")) *value = (double)s->launches;
     else if (!strcmp(key, "steps_done")) *value = (double)s->steps_done;
     else if (!strcmp(key, "graph_replays")) *value = (double)s->graph_replays;
+    else if (!strcmp(key, "andersen_threshold")) *value = (double)s->and_thr;
+    else if (!strcmp(key, "andersen_steps")) *value = (double)s->and_t;
     else if (!strcmp(key, "vl_builds") || !strcmp(key, "vl_steps") || !strcmp(key, "vl_overflow")) {
         int nb, ns, ovf, r = ljmd_vl_stats(s, &nb, &ns, &ovf);
         if (r) return r;

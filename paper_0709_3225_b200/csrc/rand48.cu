@@ -326,3 +326,61 @@ int ljmd_mb_velocities(md_sim *s, double T, uint64_t seed48, double *vraw, doubl
     CKL(s);
     return MD_OK;
 }
+
+// ---------------------------------------------------------------------------------------
+// Second half-kick + Andersen thermostat + KE (second half; reading R24 of DESIGN.md,
+// same draw ownership as oracle andersen_collide): after the half-kick of step t atom `id` takes the 7
+// draws starting at 7 (t N + id) of one rand48 stream, reached by skip-ahead and consumed in registers;
+// collision iff the 32 high bits of the first are < thr; the new velocity is computed in FP64.
+__global__ void __launch_bounds__(MB_T)
+k_kick_andersen(float4 *__restrict__ vel, const float4 *__restrict__ frc, const float4 *__restrict__ pos, int64_t N,
+                float hdt, double sqrtT, uint32_t thr, uint64_t seed, uint64_t t, double *__restrict__ part_ke)
+{
+    __shared__ double red[32];
+    const int64_t slot = (int64_t)blockIdx.x * MB_T + threadIdx.x;
+    double ke = 0.0;
+    if (slot < N) {
+        float4 v = vel[slot];
+        const float4 f = frc[slot];
+        v.x = fmaf(hdt, f.x, v.x);
+        v.y = fmaf(hdt, f.y, v.y);
+        v.z = fmaf(hdt, f.z, v.z);
+        const uint64_t id = (uint64_t)__float_as_int(pos[slot].w);
+        uint64_t x = r48_skip(seed, 7ull * (t * (uint64_t)N + id));
+        x = (R48_A * x + R48_C) & R48_MASK;
+        if ((uint32_t)(x >> 16) < thr) {
+            double nv[3];
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                x = (R48_A * x + R48_C) & R48_MASK;
+                const double u1 = R48Out<2>::cv(x);
+                x = (R48_A * x + R48_C) & R48_MASK;
+                const double u2 = R48Out<2>::cv(x);
+                nv[c] = sqrtT * sqrt(-2.0 * log(1.0 - u1)) * cos(6.283185307179586476925286766559 * u2);
+            }
+            v.x = (float)nv[0]; v.y = (float)nv[1]; v.z = (float)nv[2];
+        }
+        vel[slot] = v;
+        ke = 0.5 * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
+    }
+    ke = block_sum(ke, red);
+    if (threadIdx.x == 0) part_ke[blockIdx.x] = ke;
+}
+
+int ljmd_kick_andersen(md_sim *s)
+{
+    cudaStream_t st = s->stream;
+    if (!g_r48_table_ready) {
+        k_r48_init_table<<<1, 1, 0, st>>>();
+        CK(cudaGetLastError());
+        g_r48_launches++;
+        g_r48_table_ready = true;
+    }
+    const int nb = (int)((s->N + MB_T - 1) / MB_T);
+    k_kick_andersen<<<nb, MB_T, 0, st>>>(s->vel, s->frc, s->pos, s->N, s->hdtf, sqrt(s->and_T), s->and_thr, s->and_seed,
+                                         s->and_t, s->part);
+    CKL(s);
+    s->n_ke = nb;
+    s->and_t++;
+    return MD_OK;
+}

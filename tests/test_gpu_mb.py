@@ -54,3 +54,48 @@ def test_config1_pin_and_errors(b):
             with pytest.raises(b.MDError) as e:
                 s.init_velocities(*bad)
             assert e.value.code == b.MD_EINVAL
+
+
+@pytest.mark.parametrize("algo", [0, 1, 2])
+def test_andersen_thermostat_matches_the_oracle(b, algo, oracle_uniforms):
+    """30 steps with collisions (nu dt = 0.05) on config 1 against the oracle's step + andersen_collide."""
+    c1 = wl.md_system("c1_allpairs_500", oracle_uniforms)
+    N, L, T, nu, seed = c1["N"], c1["L"], 1.5, 10.0, 0x0123456789AB
+    with b.Sim(N, L) as s:
+        s.option("andersen_T", T)
+        s.option("andersen_seed", seed)
+        s.option("andersen_nu", nu)
+        thr = int(s.stat("andersen_threshold"))
+        assert thr == int(np.floor(nu * 0.005 * 2.0 ** 32))
+        s.set_state(c1["pos"], c1["vel"])
+        s.step(12, algo)
+        s.step(18, algo)                                   # the step index carries over between calls
+        assert s.stat("andersen_steps") == 30
+        p, v = s.get_state()
+        ke, pe, w = s.energies()
+    po, vo = c1["pos"].astype(np.float64), c1["vel"].astype(np.float64)
+    Fo, _, _ = oracle.forces(po, L, algo=0)
+    ncoll = 0
+    for t in range(30):
+        po, vo, Fo, (_, peo, wo) = oracle.verlet_step(po, vo, Fo, L, algo=0)
+        vo, n = oracle.andersen_collide(vo, T, thr, seed, t)
+        ncoll += n
+    assert 500 < ncoll < 1000                              # 30 x 500 x 0.05 = 750 expected
+    d = p.astype(np.float64) - po
+    d -= L * np.rint(d / L)
+    assert np.max(np.abs(d)) < 2e-5 and np.max(np.abs(v.astype(np.float64) - vo)) < 2e-4
+    assert ke == pytest.approx(oracle.kinetic_energy(vo), rel=1e-5) and pe == pytest.approx(peo, rel=1e-5)
+
+
+def test_andersen_off_is_plain_nve(b, oracle_uniforms):
+    c1 = wl.md_system("c1_allpairs_500", oracle_uniforms)
+    out = []
+    for nu in (None, 0.0):
+        with b.Sim(c1["N"], c1["L"]) as s:
+            if nu is not None:
+                s.option("andersen_T", 1.0)
+                s.option("andersen_nu", nu)
+            s.set_state(c1["pos"], c1["vel"])
+            s.step(20, 0)
+            out.append(s.get_state())
+    assert np.max(np.abs(out[0][1] - out[1][1])) < 1e-4
