@@ -536,20 +536,27 @@ k_force_cell_warp(const float4 *__restrict__ lpos, const int *__restrict__ cell_
     }
 }
 
-int ljmd_forces_cell(md_sim *s)
+// Cells per row group: option "cell_group", else chosen from the mean occupancy of the grid.
+static int fc_group_cells(const md_sim *s, const Grid &g)
 {
-    const Grid &g = s->grid;
-    // cells per row group: fill the 16 filter rows on average (option "cell_group" overrides)
     int kz = s->cell_group;
     if (kz <= 0) {
         const double occ = (double)s->N / (double)g.ncells;
         // measured optimum (B200): one cell per warp from about 11 atoms per cell on, else about
         // 22 filter rows per group
         kz = (occ >= 11.0) ? 1 : (int)(22.0 / (occ > 0.5 ? occ : 0.5) + 0.5);
-        if (kz < 2 && occ < 11.0) kz = 2;
+        if (kz < 2) kz = (occ >= 11.0) ? 1 : 2;
     }
     if (kz > FC_KZ_MAX) kz = FC_KZ_MAX;
     if (kz < 1 || g.n < 8) kz = 1;                  // dz * side must stay exact in FP32 (L >= 16)
+    return kz;
+}
+
+int ljmd_forces_cell(md_sim *s)
+{
+    const Grid &g = s->grid;
+    // cells per row group: fill the 16 filter rows on average (option "cell_group" overrides)
+    const int kz = fc_group_cells(s, g);
     const int nzu = (g.n + kz - 1) / kz;
     const dim3 grid((nzu + FC_WARPS - 1) / FC_WARPS, g.n, g.n);
     const int64_t nunits = (int64_t)grid.x * FC_WARPS * g.n * g.n;
@@ -595,14 +602,7 @@ int ljmd_forces_cell(md_sim *s)
 int ljmd_vl_build_lists(md_sim *s, const int *cond)
 {
     const Grid &g = s->vgrid;
-    int kz = s->cell_group;
-    if (kz <= 0) {
-        const double occ = (double)s->N / (double)g.ncells;
-        kz = (occ >= 11.0) ? 1 : (int)(22.0 / (occ > 0.5 ? occ : 0.5) + 0.5);
-        if (kz < 2 && occ < 11.0) kz = 2;
-    }
-    if (kz > FC_KZ_MAX) kz = FC_KZ_MAX;
-    if (kz < 1 || g.n < 8) kz = 1;
+    const int kz = fc_group_cells(s, g);
     const int nzu = (g.n + kz - 1) / kz;
     const dim3 grid((nzu + FC_WARPS - 1) / FC_WARPS, g.n, g.n);
     const double rl = s->rc + s->skin;
