@@ -312,3 +312,27 @@ def test_graph_replay_equals_direct_launches(b, c1, algo, opts, nsteps):
     # the counting sort's atomic ranks make the summation order run-dependent: equal up to rounding
     assert np.max(np.abs(p1 - p0)) < 1e-5 and np.max(np.abs(v1 - v0)) < 1e-4
     assert e1 == pytest.approx(e0, rel=2e-6)             # the virial is the most sensitive of the three
+
+
+@pytest.mark.parametrize("algo", [0, 1, 2])
+def test_user_stream_with_graph_replay(b, c1, algo):
+    """md_set_stream with a non-default (non-blocking) stream: graphs are captured on that stream itself."""
+    import torch
+    ref = None
+    for use_stream in (False, True):
+        with b.Sim(c1["N"], c1["L"]) as s:
+            if use_stream:
+                st = torch.cuda.Stream()
+                b.md_set_stream(s.h, st.cuda_stream)
+            s.set_state(c1["pos"], c1["vel"])
+            s.step(40, algo)
+            s.step(40, algo)
+            assert s.stat("graph_replays") > 0
+            res = (s.get_state(), s.energies())
+            if use_stream:
+                b.md_set_stream(s.h, 0)
+        if ref is None:
+            ref = res
+    d = res[0][0] - ref[0][0]
+    d -= c1["L"] * np.rint(d / c1["L"])
+    assert np.max(np.abs(d)) < 5e-5 and res[1][0] + res[1][1] == pytest.approx(ref[1][0] + ref[1][1], rel=1e-6)
