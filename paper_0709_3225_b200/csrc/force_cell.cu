@@ -21,7 +21,9 @@
 #include "common.cuh"
 #include "pair.cuh"
 
-#define FC_WARPS 4
+#ifndef FC_WARPS
+#define FC_WARPS 2                    // warps (row groups) per block: 2 wastes the fewest slots at the end of a z-column
+#endif
 #define FC_T (FC_WARPS * 32)
 #ifndef FC_CAP
 #define FC_CAP 544                    // staged candidates per pass (27 list cells of 18.5 atoms fit)
@@ -33,7 +35,7 @@
 #endif
 #define FC_NSEG ((9 * (FC_KZ_MAX + 2) + 2 + 3) & ~3)   // multiple of 4: keeps the arrays behind it 16-byte aligned
 #ifndef FC_MINB
-#define FC_MINB 4
+#define FC_MINB 8                     // blocks per SM: 16 resident warps of 128 registers
 #endif
 #define FULLMASK 0xffffffffu
 
@@ -621,7 +623,7 @@ int ljmd_vl_build_lists(md_sim *s, const int *cond)
     LO.overflow = &s->vl_ctl->overflow;
     LO.npad = s->vl_npad;
     LO.cap = s->vl_cap;
-    int nblk = (int)(grid.x * grid.y * grid.z), nres = 4 * 148 * 2;           // a few resident waves of blocks
+    int nblk = (int)(grid.x * grid.y * grid.z), nres = (16 / FC_WARPS) * 148 * 2;   // two resident waves of blocks
     if (nblk > nres) nblk = nres;
     k_force_cell_warp<false, true><<<nblk, FC_T, 0, s->stream>>>(s->lpos, s->cell_start, g, s->pp, K, s->frc, nullptr, nullptr, LO, cond);
     CKL(s);
