@@ -3,7 +3,7 @@
 // through shared memory in tiles shared by the block.  Every one of the N^2 ordered pair
 // distances is computed; what differs from the paper's G80 kernel:
 //   * the inner loop is an FP32 distance FILTER in 3 FFMA per pair: atoms are sorted along a
-//     Hilbert curve, a block owns 128 R consecutive atoms, and every chunk of 32 j atoms is
+//     Hilbert curve, a block (one warp) owns 32 R consecutive atoms, and every chunk of 32 j atoms is
 //     staged (per warp, no block barrier) already shifted to the periodic image nearest the
 //     block's centre c, so the minimum image leaves the inner loop and
 //     r^2 - |u_i|^2 = |u_j|^2 - 2 u_i.u_j  (u = x - c);
@@ -24,9 +24,12 @@
 #include "common.cuh"
 #include "pair.cuh"
 
-#define AP_T 128      // threads per block
+#define AP_T 128      // threads per block of the general kernel
+#ifndef AP_FT
+#define AP_FT 32      // threads per block of the sorted filter kernel: one warp (a block retires with its warp)
+#endif
 #define AP_TJ 32      // j atoms per staged chunk: one per lane
-#define AP_BPS 5      // resident filter blocks per SM (register bound, R = 8)
+#define AP_BPS (5 * 128 / AP_FT)   // resident filter blocks per SM (register bound, R = 8: 20 warps)
 #define AP_ET 256     // threads per block of the list evaluation kernel (32 atoms)
 #define FULLMASK 0xffffffffu
 
@@ -163,16 +166,16 @@ __device__ __forceinline__ void ap_exact(const PairParams &P, const float4 &pi, 
 }
 
 template <int R>
-__global__ void __launch_bounds__(AP_T, 5)
+__global__ void __launch_bounds__(AP_FT, AP_BPS)
 k_allpairs_filter(const float4 *__restrict__ pos, int N, float rc, float rc2, float L, float invL, float hmax,
                   int nchunks_j, int *__restrict__ nbr_count, int *__restrict__ nbr_list, int cap)
 {
-    __shared__ float4 tile[(AP_T / 32) * 2 * AP_TJ];                    // [4 warps][2][AP_TJ]
-    __shared__ float bb[(AP_T / 32) * 6];
+    __shared__ float4 tile[(AP_FT / 32) * 2 * AP_TJ];                    // [4 warps][2][AP_TJ]
+    __shared__ float bb[(AP_FT / 32) * 6];
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int split = blockIdx.y, nsplit = gridDim.y;
-    const int bbase = blockIdx.x * (AP_T * R);
+    const int bbase = blockIdx.x * (AP_FT * R);
     const int i0 = bbase + wid * (32 * R) + lane;                        // atom r of this lane: i0 + 32 r
 
     // ---- block geometry: periodic bounding box of the block's atoms.  Per dimension, a
@@ -207,7 +210,7 @@ k_allpairs_filter(const float4 *__restrict__ pos, int N, float rc, float rc2, fl
     for (int d = 0; d < 3; d++) {
         unsigned m = 0u;
 #pragma unroll
-        for (int k = 0; k < AP_T / 32; k++) m |= bbu[k * 3 + d];
+        for (int k = 0; k < AP_FT / 32; k++) m |= bbu[k * 3 + d];
         unsigned e = ~m, last = e;
         int len = 0;
         while (e) {                                  // bit i of e: bins i .. i+len all empty (cyclic)
@@ -248,7 +251,7 @@ k_allpairs_filter(const float4 *__restrict__ pos, int N, float rc, float rc2, fl
     for (int d = 0; d < 3; d++) {
         mn[d] = bb[d]; mx[d] = bb[3 + d];
 #pragma unroll
-        for (int k = 1; k < AP_T / 32; k++) {
+        for (int k = 1; k < AP_FT / 32; k++) {
             mn[d] = fminf(mn[d], bb[k * 6 + d]);
             mx[d] = fmaxf(mx[d], bb[k * 6 + 3 + d]);
         }
@@ -496,7 +499,7 @@ static int ap_sm_count()
 // i blocks and j splits for R atoms per thread: one wave of AP_BPS resident blocks per SM
 static void ap_shape(int64_t N, int R, int *iblocks, int *tsplit)
 {
-    const int ib = (int)((N + 128 * R - 1) / (128 * R));
+    const int ib = (int)((N + AP_FT * R - 1) / (AP_FT * R));
     const int ntj = (int)((N + AP_TJ - 1) / AP_TJ);
     int k = (AP_BPS * ap_sm_count()) / ib;
     if (k > ntj / 4) k = ntj / 4;                                   // at least 4 chunks per warp
@@ -534,9 +537,9 @@ void ljmd_ap_plan(md_sim *s)
     // turns out not to fit falls back to per-pair minimum images inside the kernel
     const double vol_per_atom = L * L * L / (double)s->N;
     for (int R = 8; R >= 1; R >>= 1) {
-        double side = cbrt(128.0 * R * vol_per_atom);
+        double side = cbrt((double)AP_FT * R * vol_per_atom);
         double h = 0.5 * side * 1.2 + 0.5 * L / (double)(1 << bits) + 0.3;   // 0.3: drift between re-sorts
-        if (h <= s->ap_hmax && s->N >= 128 * R) { ljmd_ap_set_R(s, R); break; }
+        if (h <= s->ap_hmax && s->N >= AP_FT * R) { ljmd_ap_set_R(s, R); break; }
     }
 }
 
@@ -563,7 +566,7 @@ static int ap_launch(md_sim *s)
 {
     const int N = (int)s->N;
     dim3 grid(s->ap_ntiles, s->ap_tsplit);
-    k_allpairs_filter<R><<<grid, AP_T, 0, s->stream>>>(s->pos, N, (float)s->rc, (float)(s->rc * s->rc), s->Lf, 1.0f / s->Lf,
+    k_allpairs_filter<R><<<grid, AP_FT, 0, s->stream>>>(s->pos, N, (float)s->rc, (float)(s->rc * s->rc), s->Lf, 1.0f / s->Lf,
                                                       s->ap_hmax, (N + AP_TJ - 1) / AP_TJ, s->nbr_count, s->nbr_list,
                                                       s->nbr_cap);
     CKL(s);
