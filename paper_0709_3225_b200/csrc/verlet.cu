@@ -19,7 +19,9 @@
 #include "common.cuh"
 #include "pair.cuh"
 
+#ifndef VL_T
 #define VL_T 128                      // threads per block of the list and force kernels
+#endif
 #define VL_Q 10                       // queued FP64 pairs per thread
 #ifndef VL_U
 #define VL_U 4                        // list entries (gathers) in flight per thread
@@ -236,10 +238,8 @@ k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams 
     __shared__ float4 offt[128];
     __shared__ unsigned queue[VL_Q][VL_T];
     __shared__ double red[32];
-    if (threadIdx.x < 125) {
-        const int t = threadIdx.x;
+    for (int t = threadIdx.x; t < 125; t += VL_T)
         offt[t] = make_float4(vl_code_value(t % 5, g), vl_code_value((t / 5) % 5, g), vl_code_value(t / 25, g), 0.f);
-    }
     __syncthreads();
     const int i = blockIdx.x * VL_T + threadIdx.x;
     double pe = 0.0, w = 0.0;
