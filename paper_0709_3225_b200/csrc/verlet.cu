@@ -22,7 +22,9 @@
 #ifndef VL_T
 #define VL_T 128                      // threads per block of the list and force kernels
 #endif
+#ifndef VL_Q
 #define VL_Q 10                       // queued FP64 pairs per thread
+#endif
 #ifndef VL_U
 #define VL_U 4                        // list entries (gathers) in flight per thread
 #endif
@@ -416,6 +418,16 @@ int ljmd_forces_verlet(md_sim *s)
     K.sig2 = P.sig2f;
     K.eps24 = P.eps24f;
     K.eps48 = 2.0f * P.eps24f;
+    {
+        // the kernel is bound by its gathers: leave the unified L1 / shared memory mostly to the L1
+        // (30 % still holds eight blocks' tables and queues); measured 3 % faster than the default split
+        static bool carved = false;
+        if (!carved) {
+            cudaFuncSetAttribute(k_vl_force<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
+            cudaFuncSetAttribute(k_vl_force<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
+            carved = true;
+        }
+    }
     if (P.mode == 2)
         k_vl_force<true><<<nbl, VL_T, 0, s->stream>>>(s->lpos, N, s->vl_npad, g, P, K, s->vl_list, s->vl_count, s->frc, ppe, pw);
     else
