@@ -133,6 +133,7 @@ struct md_sim {
     uint64_t and_seed, and_t;     // stream start state, steps since it was (re)configured
     bool precise_r2_user;         // "precise_r2" was set through md_set_option
     int cell_group;               // cells per row group of the cell-force kernel; 0 = automatic
+    int cell_kernel;              // 2 (default): force_cell2.cu; 1: the first kernel (force_cell.cu)
     int64_t launches, steps_done;
     // CUDA graphs of one "unit" of interior steps (ljmd_api.cu): the unit is the number of steps after
     // which the host-side state (buffer roles, re-sort phase) repeats, so the graph can be replayed
@@ -174,6 +175,7 @@ int ljmd_forces_verlet(md_sim *s);
 int ljmd_vl_stats(md_sim *s, int *nbuilds, int *nsteps, int *overflow);
 int ljmd_cell_build(md_sim *s);
 int ljmd_forces_cell(md_sim *s);
+int ljmd_forces_cell2(md_sim *s, bool energy);       // force_cell2.cu; energy = false: forces only
 
 // ---- small device helpers --------------------------------------------------------
 // Wrap x into [0,L) after a drift of less than L (R14): a result that rounds to L becomes 0.

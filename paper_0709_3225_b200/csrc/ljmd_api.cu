@@ -215,6 +215,7 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->use_graph = true;
     s->sort_every = 10;
     s->skin = 0.3 * sigma;
+    s->cell_kernel = 2;
     setup_grid(s);
     setup_pair(s);
 
@@ -417,7 +418,8 @@ static int check_algo(md_sim *s, int algo)
     return MD_OK;
 }
 
-static int eval_forces(md_sim *s, int algo)
+// energy = false: forces only (PE and the virial of this evaluation can never be read: an interior step of md_step)
+static int eval_forces(md_sim *s, int algo, bool energy = true)
 {
     int r;
     if (algo == MD_VERLET) {
@@ -425,7 +427,7 @@ static int eval_forces(md_sim *s, int algo)
     } else if (algo == MD_CELL) {
         if ((r = ljmd_cell_build(s))) return r;
         ljmd_tick(s, TAG_BUILD);
-        if ((r = ljmd_forces_cell(s))) return r;
+        if ((r = (s->cell_kernel == 1) ? ljmd_forces_cell(s) : ljmd_forces_cell2(s, energy))) return r;
     } else {
         if ((r = ljmd_forces_allpairs(s))) return r;
     }
@@ -441,7 +443,7 @@ static int one_step(md_sim *s, int algo, int kicks, bool last)
                                : (algo == MD_VERLET) ? ljmd_vl_kick_drift(s, kicks) : ljmd_kick_drift(s, kicks)))
         return r;
     ljmd_tick(s, TAG_INTEGRATE);
-    if ((r = eval_forces(s, algo))) return r;
+    if ((r = eval_forces(s, algo, last))) return r;
     if (last) {
         if ((r = ljmd_kick_ke(s))) return r;
         ljmd_tick(s, TAG_INTEGRATE);
@@ -658,6 +660,9 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
     } else if (!strcmp(key, "cell_group")) {
         if (value < 0 || value > 5) return MD_EINVAL;
         s->cell_group = (int)value;
+    } else if (!strcmp(key, "cell_kernel")) {
+        if (value != 1 && value != 2) return MD_EINVAL;
+        s->cell_kernel = (int)value;
     } else if (!strcmp(key, "sort_every")) {
         if (value < 1) return MD_EINVAL;
         s->sort_every = (int)value;
