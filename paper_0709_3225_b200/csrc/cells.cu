@@ -7,15 +7,6 @@
 
 #define CB_T 256
 
-__device__ __forceinline__ int cell_coord(float x, const Grid &g)
-{
-    int c = min((int)(x * g.inv_side), g.n - 1);
-    float o = (float)c * g.side;                       // exact: a multiple of the grid quantum
-    if (x < o) c--;
-    else if (c < g.n - 1 && x >= o + g.side) c++;
-    return c;
-}
-
 // Histogram with the rank inside the cell returned by the atomic.
 __global__ void __launch_bounds__(CB_T)
 k_bin(const float4 *__restrict__ pos, int N, Grid g, int *__restrict__ cell_of, int *__restrict__ rank,
@@ -251,6 +242,106 @@ int ljmd_cell_build(md_sim *s)
     CKL(s);
     float4 *t = s->pos; s->pos = s->pos2; s->pos2 = t;
     t = s->vel; s->vel = s->vel2; s->vel2 = t;
+    s->layout = LAYOUT_CELL;
+    return MD_OK;
+}
+
+// ---- lean build (force_cell2.cu, force_cell3.cu): the rank returned by the histogram's atomic rides in vel.w,
+// the scatter recomputes the cell from the position: no cell_of/rank arrays (16 B/atom less traffic), and the
+// histogram can ride in the epilogue of the force kernel (option "fuse_integrator").
+__global__ void __launch_bounds__(CB_T)
+k_bin3(const float4 *__restrict__ pos, float4 *__restrict__ vel, int N, Grid g, int *__restrict__ cell_count)
+{
+    int i = blockIdx.x * CB_T + threadIdx.x;
+    if (i >= N) return;
+    const float4 p = pos[i];
+    const int c = (cell_coord(p.x, g) * g.n + cell_coord(p.y, g)) * g.n + cell_coord(p.z, g);
+    reinterpret_cast<int *>(vel)[4 * i + 3] = atomicAdd(&cell_count[c], 1);
+}
+
+template <int KICKS>
+__global__ void __launch_bounds__(CB_T)
+k_kick_drift_bin3(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4 *__restrict__ frc, int N,
+                  float hdt, float dt, Grid g, int *__restrict__ cell_count)
+{
+    int i = blockIdx.x * CB_T + threadIdx.x;
+    if (i >= N) return;
+    float4 p = pos[i], v = vel[i];
+    const float4 f = frc[i];
+#pragma unroll
+    for (int k = 0; k < KICKS; k++) {
+        v.x = fmaf(hdt, f.x, v.x);
+        v.y = fmaf(hdt, f.y, v.y);
+        v.z = fmaf(hdt, f.z, v.z);
+    }
+    p.x = wrap_drift(fmaf(dt, v.x, p.x), g.L);
+    p.y = wrap_drift(fmaf(dt, v.y, p.y), g.L);
+    p.z = wrap_drift(fmaf(dt, v.z, p.z), g.L);
+    const int c = (cell_coord(p.x, g) * g.n + cell_coord(p.y, g)) * g.n + cell_coord(p.z, g);
+    v.w = __int_as_float(atomicAdd(&cell_count[c], 1));
+    pos[i] = p;
+    vel[i] = v;
+}
+
+__global__ void __launch_bounds__(CB_T)
+k_scatter3(const float4 *__restrict__ pos, const float4 *__restrict__ vel, int N, Grid g,
+           const int *__restrict__ cell_start, float4 *__restrict__ pos2, float4 *__restrict__ vel2,
+           float4 *__restrict__ lpos)
+{
+    int i = blockIdx.x * CB_T + threadIdx.x;
+    if (i >= N) return;
+    const float4 p = pos[i];
+    float4 v = vel[i];
+    const int c = (cell_coord(p.x, g) * g.n + cell_coord(p.y, g)) * g.n + cell_coord(p.z, g);
+    const int dst = cell_start[c] + __float_as_int(v.w);
+    v.w = 0.f;
+    pos2[dst] = p;
+    vel2[dst] = v;
+    if (lpos) {                                        // cell-local copy for the filter kernels (force_cell2.cu)
+        const int cz = c % g.n, cy = (c / g.n) % g.n, cx = c / (g.n * g.n);
+        lpos[dst] = make_float4(p.x - (float)cx * g.side, p.y - (float)cy * g.side, p.z - (float)cz * g.side,
+                                __int_as_float(c));    // exact
+    }
+}
+
+int ljmd_kick_drift_bin3(md_sim *s, int kicks)
+{
+    int N = (int)s->N;
+    int nb = (N + CB_T - 1) / CB_T;
+    if (kicks == 2)
+        k_kick_drift_bin3<2><<<nb, CB_T, 0, s->stream>>>(s->pos, s->vel, s->frc, N, s->hdtf, s->dtf, s->grid, s->cell_count);
+    else
+        k_kick_drift_bin3<1><<<nb, CB_T, 0, s->stream>>>(s->pos, s->vel, s->frc, N, s->hdtf, s->dtf, s->grid, s->cell_count);
+    CKL(s);
+    s->binned3 = true;
+    return MD_OK;
+}
+
+// Scan + scatter.  After a fused force kernel (s->fused_pending) the drifted positions are in pos2 and the
+// kicked velocities (with ranks) in vel; otherwise pos/vel hold the state, histogrammed or not.
+int ljmd_cell_build3(md_sim *s)
+{
+    int N = (int)s->N;
+    int nb = (N + CB_T - 1) / CB_T;
+    const bool pending = s->fused_pending;
+    float4 *lp = (s->cell_kernel == 3) ? nullptr : s->lpos;      // the dense kernel reads the positions as stored
+    if (!pending && !s->binned3) {
+        k_bin3<<<nb, CB_T, 0, s->stream>>>(s->pos, s->vel, N, s->grid, s->cell_count);
+        CKL(s);
+    }
+    s->binned3 = false;
+    s->fused_pending = false;
+    int r = ljmd_scan_counts(s, s->cell_count, s->cell_start, s->grid.ncells);
+    if (r) return r;
+    if (pending) {
+        k_scatter3<<<nb, CB_T, 0, s->stream>>>(s->pos2, s->vel, N, s->grid, s->cell_start, s->pos, s->vel2, lp);
+        CKL(s);
+    } else {
+        k_scatter3<<<nb, CB_T, 0, s->stream>>>(s->pos, s->vel, N, s->grid, s->cell_start, s->pos2, s->vel2, lp);
+        CKL(s);
+        float4 *t = s->pos; s->pos = s->pos2; s->pos2 = t;
+    }
+    float4 *t = s->vel; s->vel = s->vel2; s->vel2 = t;
     s->layout = LAYOUT_CELL;
     return MD_OK;
 }

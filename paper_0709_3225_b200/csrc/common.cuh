@@ -124,6 +124,8 @@ struct md_sim {
     int layout;                   // LAYOUT_*: how the slots are currently ordered
     bool has_state, forces_valid;
     bool binned;                  // cell_of/rank/cell_count already hold the histogram of the current positions
+    bool binned3;                 // lean build: vel.w/cell_count hold the histogram of the current positions
+    bool fused_pending;           // the last force kernel integrated: pos2 = drifted positions, vel = kicked velocities with ranks in .w
     int forces_algo;
     bool use_graph;
     int sort_every;
@@ -133,7 +135,8 @@ struct md_sim {
     uint64_t and_seed, and_t;     // stream start state, steps since it was (re)configured
     bool precise_r2_user;         // "precise_r2" was set through md_set_option
     int cell_group;               // cells per row group of the cell-force kernel; 0 = automatic
-    int cell_kernel;              // 2 (default): force_cell2.cu; 1: the first kernel (force_cell.cu)
+    int cell_kernel;              // 2 (default): force_cell2.cu; 3: force_cell3.cu (dense); 1: force_cell.cu
+    bool fuse_integrator;         // option "fuse_integrator": interior steps integrate in the force kernel's epilogue
     int64_t launches, steps_done;
     // CUDA graphs of one "unit" of interior steps (ljmd_api.cu): the unit is the number of steps after
     // which the host-side state (buffer roles, re-sort phase) repeats, so the graph can be replayed
@@ -175,7 +178,10 @@ int ljmd_forces_verlet(md_sim *s);
 int ljmd_vl_stats(md_sim *s, int *nbuilds, int *nsteps, int *overflow);
 int ljmd_cell_build(md_sim *s);
 int ljmd_forces_cell(md_sim *s);
-int ljmd_forces_cell2(md_sim *s, bool energy);       // force_cell2.cu; energy = false: forces only
+int ljmd_forces_cell2(md_sim *s, bool energy, bool fused);   // force_cell2.cu; energy = false: forces only; fused: the epilogue integrates
+int ljmd_forces_cell3(md_sim *s, bool energy, bool fused);   // force_cell3.cu; fused: the epilogue integrates
+int ljmd_kick_drift_bin3(md_sim *s, int kicks);      // cells.cu: lean build (rank in vel.w)
+int ljmd_cell_build3(md_sim *s);
 
 // ---- small device helpers --------------------------------------------------------
 // Wrap x into [0,L) after a drift of less than L (R14): a result that rounds to L becomes 0.
@@ -185,6 +191,17 @@ __device__ __forceinline__ float wrap_drift(float x, float L)
     else if (x < 0.0f) x += L;
     if (x >= L || x < 0.0f) x = 0.0f;
     return x;
+}
+
+// Cell index of coordinate x in [0,L) (cells 0..n-2 of width side, the last one takes the remainder):
+// the reciprocal multiply is corrected against the exact cell origins.
+__device__ __forceinline__ int cell_coord(float x, const Grid &g)
+{
+    int c = min((int)(x * g.inv_side), g.n - 1);
+    float o = (float)c * g.side;                       // exact: a multiple of the grid quantum
+    if (x < o) c--;
+    else if (c < g.n - 1 && x >= o + g.side) c++;
+    return c;
 }
 
 __device__ __forceinline__ double warp_sum(double v)

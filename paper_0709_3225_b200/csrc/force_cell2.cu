@@ -53,6 +53,7 @@ struct F2Const {
     double hd;
     int nzu;
     int tile_exact;                   // the staged FP32 coordinates are exact for warps away from the box origin
+    float hdt, dt;                    // fused integrator
 };
 
 __device__ __forceinline__ int f2_bfind(unsigned x)      // index of the highest set bit, -1 for 0
@@ -167,11 +168,16 @@ __device__ __forceinline__ void f2_filter(const float *__restrict__ tx, const fl
     }
 }
 
-template <int KK, bool MODE2, bool ENERGY>
+// FUSED: the lane that owns F_i also applies the closing half-kick of this step and the opening half-kick,
+// drift, wrap and cell histogram of the next one (the arithmetic of k_kick_drift_bin3<2>, cells.cu, on the
+// float force), writing the drifted positions to pos_out and the kicked velocities (rank in .w) in place:
+// an interior step of md_step is then force kernel + scan + scatter, and the forces never reach HBM.
+template <int KK, bool MODE2, bool ENERGY, bool FUSED>
 __global__ void __launch_bounds__(32, F2_MINB)
 k_fc2(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, const Grid g, const PairParams P,
       const F2Const K, float4 *__restrict__ frc, double *__restrict__ part_pe, double *__restrict__ part_w,
-      const int nmax)
+      const int nmax, const float4 *__restrict__ pos, float4 *__restrict__ vel, float4 *__restrict__ pos_out,
+      int *__restrict__ cell_count)
 {
     typedef F2Geom<KK> G;
     __shared__ __align__(16) F2Smem<KK> S;
@@ -253,6 +259,8 @@ k_fc2(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, const
             const bool myvalid = sl < SL;
             const int myslot = ibeg + i0 + li_;
             const float4 lme = lpos[myslot];
+            float4 pme4, vme4;
+            if (FUSED) { pme4 = pos[myslot]; vme4 = vel[myslot]; }   // early: the latency hides behind the pass
             float zoff_me = 0.f;
 #pragma unroll
             for (int k = 1; k < KK; k++) zoff_me += (k < kk && myslot >= cell_start[cfirst + k]) ? g.side : 0.f;
@@ -494,7 +502,25 @@ k_fc2(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, const
                         const float4 f0 = frc[myslot];
                         tx_ += (double)f0.x; ty_ += (double)f0.y; tz_ += (double)f0.z;
                     }
-                    frc[myslot] = make_float4((float)(tx_ + ox_), (float)(ty_ + oy_), (float)(tz_ + oz_), 0.f);
+                    const float fx = (float)(tx_ + ox_), fy = (float)(ty_ + oy_), fz = (float)(tz_ + oz_);
+                    if (!FUSED || t0 + F2_CAP < total) {
+                        frc[myslot] = make_float4(fx, fy, fz, 0.f);
+                    } else {
+                        float4 p = pme4, v = vme4;
+#pragma unroll
+                        for (int k = 0; k < 2; k++) {
+                            v.x = fmaf(K.hdt, fx, v.x);
+                            v.y = fmaf(K.hdt, fy, v.y);
+                            v.z = fmaf(K.hdt, fz, v.z);
+                        }
+                        p.x = wrap_drift(fmaf(K.dt, v.x, p.x), g.L);
+                        p.y = wrap_drift(fmaf(K.dt, v.y, p.y), g.L);
+                        p.z = wrap_drift(fmaf(K.dt, v.z, p.z), g.L);
+                        const int c = (cell_coord(p.x, g) * n + cell_coord(p.y, g)) * n + cell_coord(p.z, g);
+                        v.w = __int_as_float(atomicAdd(&cell_count[c], 1));   // rank inside the new cell
+                        pos_out[myslot] = p;
+                        vel[myslot] = v;
+                    }
                 }
                 if (ENERGY) {
                     // PE = 4 eps (A - B) - n ushift [+ f_rc sum(r - rc)],  W = 24 eps (2A - B) [- f_rc sum r]
@@ -537,22 +563,26 @@ int ljmd_fc2_group_cells(const md_sim *s, const Grid &g)
 }
 
 template <int KK>
-static void fc2_launch(md_sim *s, const dim3 grid, const F2Const &K, double *ppe, double *pw, bool energy)
+static void fc2_launch(md_sim *s, const dim3 grid, const F2Const &K, double *ppe, double *pw, bool energy, bool fused)
 {
     const PairParams &P = s->pp;
     const int nmax = (int)s->N - 1;
-    if (P.mode == 2) {
-        if (energy) k_fc2<KK, true, true><<<grid, 32, 0, s->stream>>>(s->lpos, s->cell_start, s->grid, P, K, s->frc, ppe, pw, nmax);
-        else k_fc2<KK, true, false><<<grid, 32, 0, s->stream>>>(s->lpos, s->cell_start, s->grid, P, K, s->frc, ppe, pw, nmax);
+#define F2_LAUNCH(M2, EN, FU) \
+    k_fc2<KK, M2, EN, FU><<<grid, 32, 0, s->stream>>>(s->lpos, s->cell_start, s->grid, P, K, s->frc, ppe, pw, nmax, s->pos, s->vel, s->pos2, s->cell_count)
+    if (fused) {                                    // interior steps: forces only
+        if (P.mode == 2) F2_LAUNCH(true, false, true); else F2_LAUNCH(false, false, true);
+    } else if (P.mode == 2) {
+        if (energy) F2_LAUNCH(true, true, false); else F2_LAUNCH(true, false, false);
     } else {
-        if (energy) k_fc2<KK, false, true><<<grid, 32, 0, s->stream>>>(s->lpos, s->cell_start, s->grid, P, K, s->frc, ppe, pw, nmax);
-        else k_fc2<KK, false, false><<<grid, 32, 0, s->stream>>>(s->lpos, s->cell_start, s->grid, P, K, s->frc, ppe, pw, nmax);
+        if (energy) F2_LAUNCH(false, true, false); else F2_LAUNCH(false, false, false);
     }
+#undef F2_LAUNCH
 }
 
 // energy = false: forces only (interior steps of md_step, whose PE and virial nobody can read)
-int ljmd_forces_cell2(md_sim *s, bool energy)
+int ljmd_forces_cell2(md_sim *s, bool energy, bool fused)
 {
+    if (fused) energy = false;
     const Grid &g = s->grid;
     const int kz = ljmd_fc2_group_cells(s, g);
     const int nzu = (g.n + kz - 1) / kz;
@@ -584,14 +614,17 @@ int ljmd_forces_cell2(md_sim *s, bool energy)
     K.neps48 = -2.0f * P.eps24f;
     K.f_rcf = P.f_rcf;
     K.rcf = P.rcf;
+    K.hdt = s->hdtf;
+    K.dt = s->dtf;
     switch (kz) {
-    case 1: fc2_launch<1>(s, grid, K, ppe, pw, energy); break;
-    case 2: fc2_launch<2>(s, grid, K, ppe, pw, energy); break;
-    case 3: fc2_launch<3>(s, grid, K, ppe, pw, energy); break;
-    default: fc2_launch<5>(s, grid, K, ppe, pw, energy); break;
+    case 1: fc2_launch<1>(s, grid, K, ppe, pw, energy, fused); break;
+    case 2: fc2_launch<2>(s, grid, K, ppe, pw, energy, fused); break;
+    case 3: fc2_launch<3>(s, grid, K, ppe, pw, energy, fused); break;
+    default: fc2_launch<5>(s, grid, K, ppe, pw, energy, fused); break;
     }
     CKL(s);
     ljmd_tick(s, TAG_FORCE);
     if (energy) s->n_pe = (int)nunits;
+    if (fused) s->fused_pending = true;
     return MD_OK;
 }

@@ -332,6 +332,8 @@ extern "C" int md_set_state(md_sim *s, const float *pos, const float *vel)
     CK(cudaStreamSynchronize(s->stream));
     s->has_state = true;
     s->binned = false;
+    s->binned3 = false;
+    s->fused_pending = false;
     s->forces_valid = false;
     s->layout = LAYOUT_NONE;
     return MD_OK;
@@ -419,15 +421,21 @@ static int check_algo(md_sim *s, int algo)
 }
 
 // energy = false: forces only (PE and the virial of this evaluation can never be read: an interior step of md_step)
-static int eval_forces(md_sim *s, int algo, bool energy = true)
+// fuse = true (dense cell kernel only): the force kernel's epilogue also integrates up to the next step's
+// histogram (force_cell3.cu), and the next one_step starts at the scan
+static int eval_forces(md_sim *s, int algo, bool energy = true, bool fuse = false)
 {
     int r;
     if (algo == MD_VERLET) {
         if ((r = ljmd_forces_verlet(s))) return r;
+    } else if (algo == MD_CELL && s->cell_kernel >= 2) {
+        if ((r = ljmd_cell_build3(s))) return r;
+        ljmd_tick(s, TAG_BUILD);
+        if ((r = (s->cell_kernel == 3) ? ljmd_forces_cell3(s, energy, fuse) : ljmd_forces_cell2(s, energy, fuse))) return r;
     } else if (algo == MD_CELL) {
         if ((r = ljmd_cell_build(s))) return r;
         ljmd_tick(s, TAG_BUILD);
-        if ((r = (s->cell_kernel == 1) ? ljmd_forces_cell(s) : ljmd_forces_cell2(s, energy))) return r;
+        if ((r = ljmd_forces_cell(s))) return r;
     } else {
         if ((r = ljmd_forces_allpairs(s))) return r;
     }
@@ -436,14 +444,19 @@ static int eval_forces(md_sim *s, int algo, bool energy = true)
 
 // One velocity-Verlet step: [pending half-kick +] half-kick + drift [+ histogram], forces,
 // and on the last step of a call the closing half-kick + KE.
-static int one_step(md_sim *s, int algo, int kicks, bool last)
+// energy: PE and the virial of this evaluation will be read.  may_fuse = false keeps the integrator out of the
+// force kernel (the thermostat changes the velocities between the two half-kicks).
+static int one_step(md_sim *s, int algo, int kicks, bool last, bool energy, bool may_fuse = true)
 {
     int r;
-    if ((r = (algo == MD_CELL) ? ljmd_kick_drift_bin(s, kicks)
-                               : (algo == MD_VERLET) ? ljmd_vl_kick_drift(s, kicks) : ljmd_kick_drift(s, kicks)))
-        return r;
-    ljmd_tick(s, TAG_INTEGRATE);
-    if ((r = eval_forces(s, algo, last))) return r;
+    const bool k3 = algo == MD_CELL && s->cell_kernel >= 2;      // lean build, fusable force kernel
+    if (!(k3 && s->fused_pending)) {                   // else: the previous force kernel has integrated already
+        if ((r = (algo == MD_CELL) ? (k3 ? ljmd_kick_drift_bin3(s, kicks) : ljmd_kick_drift_bin(s, kicks))
+                                   : (algo == MD_VERLET) ? ljmd_vl_kick_drift(s, kicks) : ljmd_kick_drift(s, kicks)))
+            return r;
+        ljmd_tick(s, TAG_INTEGRATE);
+    }
+    if ((r = eval_forces(s, algo, energy, k3 && !last && may_fuse && s->fuse_integrator))) return r;
     if (last) {
         if ((r = ljmd_kick_ke(s))) return r;
         ljmd_tick(s, TAG_INTEGRATE);
@@ -501,7 +514,7 @@ static int replay_interior(md_sim *s, int algo, int unit, int64_t nunits, int64_
         int r = MD_OK;
         if (cudaStreamBeginCapture(run, cudaStreamCaptureModeThreadLocal) != cudaSuccess) r = MD_ECUDA;
         if (r == MD_OK) {
-            for (int q = 0; q < unit && r == MD_OK; q++) r = one_step(s, algo, 2, false);
+            for (int q = 0; q < unit && r == MD_OK; q++) r = one_step(s, algo, 2, false, false);
             cudaError_t ce = cudaStreamEndCapture(run, &graph);
             if (ce != cudaSuccess || !graph) r = MD_ECUDA;
         }
@@ -580,7 +593,7 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
         // Andersen thermostat: the collisions follow every second half-kick, so nothing is folded into
         // the next step and the step index is a kernel argument (direct launches, no graph)
         for (; k < nsteps; k++) {
-            if ((r = one_step(s, algo, 1, false))) return r;
+            if ((r = one_step(s, algo, 1, false, k == nsteps - 1, false))) return r;
             if ((r = ljmd_kick_andersen(s))) return r;
             ljmd_tick(s, TAG_INTEGRATE);
         }
@@ -595,7 +608,7 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
                 if (done) continue;
             }
         }
-        if ((r = one_step(s, algo, (k > 0) ? 2 : 1, k == nsteps - 1))) return r;
+        if ((r = one_step(s, algo, (k > 0) ? 2 : 1, k == nsteps - 1, k == nsteps - 1))) return r;
         k++;
     }
     if ((r = ljmd_reduce_energies(s))) return r;
@@ -660,8 +673,10 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
     } else if (!strcmp(key, "cell_group")) {
         if (value < 0 || value > 5) return MD_EINVAL;
         s->cell_group = (int)value;
+    } else if (!strcmp(key, "fuse_integrator")) {
+        s->fuse_integrator = value != 0.0;
     } else if (!strcmp(key, "cell_kernel")) {
-        if (value != 1 && value != 2) return MD_EINVAL;
+        if (value != 1 && value != 2 && value != 3) return MD_EINVAL;
         s->cell_kernel = (int)value;
     } else if (!strcmp(key, "sort_every")) {
         if (value < 1) return MD_EINVAL;
