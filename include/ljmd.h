@@ -40,8 +40,12 @@ typedef enum md_status {
 /* algo.  MD_VERLET (an extension beyond the paper's two algorithms; it discusses neighbour lists in
  * PAPER.md:100-104): neighbour lists with a skin, built from a cell list of side >= rc + skin and rebuilt,
  * on the device's own decision, whenever an atom has moved more than skin / 2 since the last build.  Same
- * forces as the other two paths; MD_EDOMAIN if int[L / (rc + skin)] < 3, MD_EUNSUPPORTED if N > 2^23 - 1,
- * MD_ENOMEM from md_step if a list overflowed its capacity (1.4 x the mean length + 32). */
+ * forces as the other two paths; MD_EDOMAIN if int[L / (rc + skin)] < 3, MD_EUNSUPPORTED if N > 2^23 - 1.
+ * Lists start with room for 1.4 x the mean length + 32 entries and are never truncated silently: a build
+ * that needs more makes md_compute_forces (and the evaluation md_step does on stale forces) reallocate them
+ * for the length asked for and rebuild; if that happens in the middle of md_step, the call returns MD_ENOMEM,
+ * the forces and the trajectory since that build are not valid (set the state again; the lists have been
+ * enlarged for the next attempt). */
 enum { MD_ALLPAIRS = 0, MD_CELL = 1, MD_VERLET = 2 };
 enum { MD_TRUNCATED = 0, MD_ENERGY_SHIFTED = 1, MD_FORCE_SHIFTED = 2 }; /* shifted */
 enum { R48_U32_HI32 = 0, R48_U32_HI31 = 1, R48_F64 = 2, R48_U64_STATE = 3 }; /* kind */
@@ -112,12 +116,16 @@ const char *md_strerror(int code);
 
 /* Stream (a cudaStream_t passed as void*) on which this handle's kernels run. */
 int md_set_stream(md_sim *s, void *cuda_stream);
-/* Stream used by rand48_fill (process-wide). */
+/* The same on an explicit CUDA stream (no process-wide state involved). */
+int rand48_fill_on(uint64_t *seeds, int64_t nstreams, int64_t ndraws, int kind, void *out, void *cuda_stream);
+
+/* Stream used by rand48_fill (process-wide; rand48_fill_on takes the stream per call instead). */
 int rand48_set_stream(void *cuda_stream);
 
 /* Device allocator hooks (process-wide), e.g. PyTorch's caching allocator.  alloc returns a
  * device pointer or NULL; both are called with the stream in use.  NULL, NULL restores
- * cudaMalloc/cudaFree.  Must be set before the handles that use them are created. */
+ * cudaMalloc/cudaFree.  May be changed at any time: every block is released through the hook
+ * that was installed when it was allocated. */
 typedef void *(*md_alloc_fn)(int64_t bytes, void *cuda_stream);
 typedef void (*md_free_fn)(void *ptr, void *cuda_stream);
 int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
@@ -143,15 +151,24 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
  *   "time_kernels"   1 = record CUDA events around every phase of md_step (disables the graph);
  *                    read back with md_get_stat "t_force_ms", "t_build_ms", "t_integrate_ms",
  *                    "t_other_ms", "n_force"; setting it resets the accumulators
- *   "precise_r2"     squared distance below which the pair term is evaluated in FP64
- *                    (default: all in-range pairs); 0 = FP32 everywhere
+ *   "precise_r2"     cell and neighbour-list paths: squared distance below which an in-range pair is
+ *                    evaluated in FP64 from the exact cell-local coordinates.  Default 1.3 sigma^2
+ *                    (1.5 sigma^2 when the cell kernel groups several cells per warp); 0 = FP32 for
+ *                    every pair but the sliver around rc^2; a huge value = FP64 for every in-range
+ *                    pair.  The all-pairs path always evaluates every in-range pair in FP64.
+ *   "cell_kernel"    cell-force kernel: 2 (default) ballot filter + per-lane walk (force_cell2.cu),
+ *                    1 its first version (force_cell.cu), 3 dense evaluation of every staged
+ *                    candidate (force_cell3.cu); same forces within the tolerances of DESIGN.md 12
+ *   "fuse_integrator" 1 = interior steps of md_step(MD_CELL) integrate in the force kernel's epilogue
+ *                    (kernels 2 and 3; default 0: measured slower)
  *   "sort_every"     all-pairs path: re-sort atoms along the Hilbert curve every k steps (default 10)
  *   "ap_general"     1 = force the unsorted per-pair-minimum-image all-pairs kernel
  *   "ap_R"           atoms per thread (1, 2, 4, 8) of the sorted all-pairs kernel, overriding the
  *                    choice made from N and L; blocks too wide for the box test per-pair images
  * md_get_stat keys: "ncell" (cells per dimension), "max_occupancy", "kernel_launches"
  * (kernels launched by this handle so far, graph nodes included), "graph_replays", "vl_builds", "vl_steps",
- * "vl_overflow", "vl_cap" (neighbour-list builds, evaluations, overflow flag, capacity), "steps_done",
+ * "vl_overflow", "vl_cap" (neighbour-list builds, evaluations, 0 or the list length the last build needed
+ * beyond the capacity, capacity), "steps_done",
  * "side" (cell side). */
 int md_set_option(md_sim *s, const char *key, double value);
 int md_get_stat(md_sim *s, const char *key, double *value);

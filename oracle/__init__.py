@@ -48,6 +48,8 @@ def lib():
         L.cell_grid.restype = i32
         L.near_cutoff_pairs.argtypes = [i64, vp, d, d, d, vp, i64]
         L.near_cutoff_pairs.restype = i64
+        L.near_cutoff_pairs_cell.argtypes = [i64, vp, d, d, d, vp, i64]
+        L.near_cutoff_pairs_cell.restype = i64
         L.kinetic_energy.argtypes = [i64, vp]
         L.kinetic_energy.restype = d
         L.verlet_step.argtypes = [i64, vp, vp, vp, d, d, d, d, d, i32, i32, pd, pd, pd]
@@ -126,6 +128,16 @@ def near_cutoff_pairs(pos, L, rc=2.5, tol=4e-7, cap=1 << 16):
     pos = _f64(pos)
     out = np.zeros((cap, 2), dtype=np.int64)
     n = lib().near_cutoff_pairs(pos.shape[0], _ptr(pos), L, rc, tol, _ptr(out), cap)
+    return out[:min(n, cap)], n
+
+
+def near_cutoff_pairs_cell(pos, L, rc=2.5, tol=4e-7, cap=1 << 16):
+    """The same ordered pairs through the linked cells (large N).  PAPER.md:98, :108; R16."""
+    pos = _f64(pos)
+    out = np.zeros((cap, 2), dtype=np.int64)
+    n = lib().near_cutoff_pairs_cell(pos.shape[0], _ptr(pos), L, rc, tol, _ptr(out), cap)
+    if n < 0:
+        raise ValueError("fewer than 3 cells per dimension")
     return out[:min(n, cap)], n
 
 

@@ -17,6 +17,7 @@ if not os.path.exists(LIB_PATH):
         "(needs nvcc).  There is no CPU fallback.")
 
 _lib = ctypes.CDLL(LIB_PATH)
+_alloc_keepalive = []
 
 MD_OK, MD_EINVAL, MD_EDOMAIN, MD_ESTATE, MD_ENOMEM, MD_ECUDA, MD_EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 MD_ALLPAIRS, MD_CELL, MD_VERLET = 0, 1, 2
@@ -39,6 +40,7 @@ _SIGS = {
     "md_get_forces": ([_vp, _vp], _i32),
     "md_get_energies": ([_vp, _pd, _pd, _pd], _i32),
     "rand48_fill": ([_vp, _i64, _i64, _i32, _vp], _i32),
+    "rand48_fill_on": ([_vp, _i64, _i64, _i32, _vp, _vp], _i32),
     "md_strerror": ([_i32], ctypes.c_char_p),
     "md_init_velocities": ([_vp, ctypes.c_double, ctypes.c_uint64], _i32),
     "md_set_stream": ([_vp, _vp], _i32),
@@ -94,9 +96,32 @@ def md_last_cuda_error():
     return _lib.md_last_cuda_error().decode()
 
 
-def md_create(N, L, rc, eps, sigma, dt, shifted):
+def _torch_cuda():
+    """torch, if it is importable and sees a device; else None (the raw C ABI needs neither)."""
+    try:
+        import torch
+    except ImportError:
+        return None
+    return torch if torch.cuda.is_available() else None
+
+
+def current_stream():
+    """Handle of PyTorch's current CUDA stream (0 = legacy default stream when torch is absent)."""
+    t = _torch_cuda()
+    return int(t.cuda.current_stream().cuda_stream) if t is not None else 0
+
+
+def md_create(N, L, rc, eps, sigma, dt, shifted, torch_plumbing=True):
+    """md_create; with torch_plumbing (default) the handle allocates through PyTorch's caching allocator
+    and runs on PyTorch's current stream, as north_star prescribes ("PyTorch is used only for device memory
+    and streams"); False leaves the library's own defaults (cudaMalloc, legacy default stream)."""
+    t = _torch_cuda() if torch_plumbing else None
+    if t is not None and not _alloc_keepalive:
+        use_torch_allocator()
     h = _vp()
     _check(_lib.md_create(ctypes.byref(h), N, L, rc, eps, sigma, dt, shifted), "md_create")
+    if t is not None:
+        md_set_stream(h, current_stream())
     return h
 
 
@@ -130,8 +155,10 @@ def md_get_energies(h):
     return ke.value, pe.value, w.value
 
 
-def rand48_fill(seeds, nstreams, ndraws, kind, out):
-    _check(_lib.rand48_fill(_addr(seeds), nstreams, ndraws, kind, _addr(out)), "rand48_fill")
+def rand48_fill(seeds, nstreams, ndraws, kind, out, stream=None):
+    """rand48_fill on `stream` (default: PyTorch's current stream)."""
+    st = current_stream() if stream is None else int(stream)
+    _check(_lib.rand48_fill_on(_addr(seeds), nstreams, ndraws, kind, _addr(out), st), "rand48_fill")
 
 
 def md_init_velocities(h, T, seed48):
@@ -158,9 +185,6 @@ def md_get_stat(h, key):
 
 def rand48_kernel_launches():
     return _lib.rand48_kernel_launches()
-
-
-_alloc_keepalive = []
 
 
 def use_torch_allocator():

@@ -66,7 +66,7 @@ struct VlCtl {
     unsigned maxd2;               // bits of the largest squared displacement since the last build
     int rebuild;                  // this step's decision (read by the build kernels)
     int force;                    // host request: build at the next evaluation
-    int overflow;                 // some list was longer than the capacity
+    int overflow;                 // 0, or the longest list length the last build needed when it exceeded the capacity
     int nbuilds, nsteps;          // statistics
 };
 
@@ -176,6 +176,7 @@ int ljmd_vl_kick_drift(md_sim *s, int kicks);
 int ljmd_vl_build_lists(md_sim *s, const int *cond);    // force_cell.cu: lists through the cell kernel's filter
 int ljmd_forces_verlet(md_sim *s);
 int ljmd_vl_stats(md_sim *s, int *nbuilds, int *nsteps, int *overflow);
+int ljmd_vl_grow(md_sim *s, int need);               // longer lists after an overflow; the next evaluation rebuilds
 int ljmd_cell_build(md_sim *s);
 int ljmd_forces_cell(md_sim *s);
 int ljmd_forces_cell2(md_sim *s, bool energy, bool fused);   // force_cell2.cu; energy = false: forces only; fused: the epilogue integrates

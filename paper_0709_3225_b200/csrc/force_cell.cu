@@ -405,7 +405,7 @@ __device__ __forceinline__ void fc_cell(FcWarp &S, const float4 *__restrict__ lp
         }
         if (LIST) {
             if (sl == 0) {
-                if (rowbase > LO.cap) *LO.overflow = 1;
+                if (rowbase > LO.cap) atomicMax(LO.overflow, rowbase);   // the length this list needs
                 int cnt = min(rowbase, LO.cap);
                 // pad to a multiple of 4 with inert entries (verlet.cu: the atom itself, displaced by a cell diagonal)
                 for (; cnt & 3; cnt++) LO.list[(size_t)cnt * LO.npad + (ibeg + i0 + li_)] = (unsigned)(ibeg + i0 + li_) | (31u << 23);

@@ -5,7 +5,9 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <mutex>
 #include <new>
+#include <unordered_map>
 #include "common.cuh"
 
 // ---- errors -------------------------------------------------------------------------
@@ -45,15 +47,29 @@ extern "C" int md_set_allocator(md_alloc_fn a, md_free_fn f)
     return MD_OK;
 }
 
+// Every block remembers the hook that has to release it (nullptr: cudaFree), so that the allocator may be
+// changed while handles created under the previous one are still alive.
+static std::mutex g_owner_mu;
+static std::unordered_map<void *, md_free_fn> g_owner;
+
 void *ljmd_dev_alloc(int64_t bytes, cudaStream_t st)
 {
     if (bytes <= 0) bytes = 16;
-    if (g_alloc) return g_alloc(bytes, (void *)st);
     void *p = nullptr;
-    cudaError_t e = cudaMalloc(&p, (size_t)bytes);
-    if (e != cudaSuccess) {
-        ljmd_note_cuda_error(e, "cudaMalloc", __FILE__, __LINE__);
-        return nullptr;
+    md_free_fn owner = nullptr;
+    if (g_alloc) {
+        p = g_alloc(bytes, (void *)st);
+        owner = g_free;
+    } else {
+        cudaError_t e = cudaMalloc(&p, (size_t)bytes);
+        if (e != cudaSuccess) {
+            ljmd_note_cuda_error(e, "cudaMalloc", __FILE__, __LINE__);
+            return nullptr;
+        }
+    }
+    if (p) {
+        std::lock_guard<std::mutex> lk(g_owner_mu);
+        g_owner[p] = owner;
     }
     return p;
 }
@@ -61,7 +77,16 @@ void *ljmd_dev_alloc(int64_t bytes, cudaStream_t st)
 void ljmd_dev_free(void *p, cudaStream_t st)
 {
     if (!p) return;
-    if (g_free) g_free(p, (void *)st);
+    md_free_fn owner = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_owner_mu);
+        auto it = g_owner.find(p);
+        if (it != g_owner.end()) {
+            owner = it->second;
+            g_owner.erase(it);
+        }
+    }
+    if (owner) owner(p, (void *)st);
     else cudaFree(p);
 }
 
@@ -553,13 +578,30 @@ static int replay_interior(md_sim *s, int algo, int unit, int64_t nunits, int64_
     return MD_OK;
 }
 
+// Force evaluation outside the step loop.  On the neighbour-list path a list longer than the capacity is
+// never silently truncated: the lists are reallocated for the length the build asked for and rebuilt.
+static int eval_forces_checked(md_sim *s, int algo)
+{
+    int r;
+    for (int attempt = 0;; attempt++) {
+        if ((r = eval_forces(s, algo))) return r;
+        if (algo != MD_VERLET) return MD_OK;
+        int nb, ns, ovf;
+        if ((r = ljmd_vl_stats(s, &nb, &ns, &ovf))) return r;
+        if (!ovf) return MD_OK;
+        s->forces_valid = false;
+        if (attempt == 3) return MD_ENOMEM;
+        if ((r = ljmd_vl_grow(s, ovf))) return r;
+    }
+}
+
 extern "C" int md_compute_forces(md_sim *s, int algo)
 {
     if (!s) return MD_EINVAL;
     if (!s->has_state) return MD_ESTATE;
     int r = check_algo(s, algo);
     if (r) return r;
-    if ((r = eval_forces(s, algo))) return r;
+    if ((r = eval_forces_checked(s, algo))) return r;
     if ((r = ljmd_ke_only(s))) return r;
     if ((r = ljmd_reduce_energies(s))) return r;
     CK(cudaStreamSynchronize(s->stream));
@@ -577,7 +619,7 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
     // the neighbour-list integrator needs the lists' local coordinates: evaluate first if another
     // path (or md_set_state) ran last
     if (!s->forces_valid || (algo == MD_VERLET && s->layout != LAYOUT_VERLET && nsteps > 0)) {
-        if ((r = eval_forces(s, algo))) return r;
+        if ((r = eval_forces_checked(s, algo))) return r;
         if ((r = ljmd_ke_only(s))) return r;
         s->forces_valid = true;
         s->forces_algo = algo;
@@ -618,7 +660,13 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
     if (algo == MD_VERLET) {
         int nb, ns, ovf;
         if ((r = ljmd_vl_stats(s, &nb, &ns, &ovf))) return r;
-        if (ovf) return MD_ENOMEM;                      // a neighbour list overflowed: results are not valid
+        if (ovf) {
+            // a list outgrew the capacity during the run: the trajectory since that build is not valid.  The
+            // lists are enlarged for the next attempt; the caller has to set the state again.
+            s->forces_valid = false;
+            ljmd_vl_grow(s, ovf);
+            return MD_ENOMEM;
+        }
     }
     s->forces_algo = algo;
     s->steps_done += nsteps;

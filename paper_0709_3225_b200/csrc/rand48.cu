@@ -128,8 +128,24 @@ k_rand48_validate(const uint64_t *__restrict__ seeds, int64_t nstreams)
 }
 
 static cudaStream_t g_r48_stream = 0;
-static bool g_r48_table_ready = false;
 static int64_t g_r48_launches = 0;
+
+// The skip-ahead table lives in __device__ memory, i.e. once per device: fill it on the first use on each
+// device, and wait for it once, since later calls may come on other streams.
+static int r48_ensure_table(cudaStream_t st)
+{
+    static bool ready[64] = {false};
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return MD_EUNSUPPORTED;
+    if (ready[dev]) return MD_OK;
+    k_r48_init_table<<<1, 1, 0, st>>>();
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(st));
+    g_r48_launches++;
+    ready[dev] = true;
+    return MD_OK;
+}
 
 extern "C" int rand48_set_stream(void *stream)
 {
@@ -151,12 +167,17 @@ static bool on_device(const void *p)
 
 extern "C" int rand48_fill(uint64_t *seeds, int64_t nstreams, int64_t ndraws, int kind, void *out)
 {
+    return rand48_fill_on(seeds, nstreams, ndraws, kind, out, (void *)g_r48_stream);
+}
+
+extern "C" int rand48_fill_on(uint64_t *seeds, int64_t nstreams, int64_t ndraws, int kind, void *out, void *stream)
+{
     if (nstreams < 0 || ndraws < 0 || kind < 0 || kind > 3) return MD_EINVAL;
     if (nstreams == 0) return MD_OK;
     if (!seeds) return MD_EINVAL;
     if (ndraws > 0 && !out) return MD_EINVAL;
     if (ndraws > (int64_t)R48_MASK) return MD_EINVAL;
-    cudaStream_t st = g_r48_stream;
+    cudaStream_t st = (cudaStream_t)stream;
     const size_t esize = (kind <= 1) ? 4 : 8;
     const bool seeds_dev = on_device(seeds);
     const bool out_dev = ndraws == 0 || on_device(out);
@@ -181,11 +202,9 @@ extern "C" int rand48_fill(uint64_t *seeds, int64_t nstreams, int64_t ndraws, in
     }
     if (ndraws == 0) return MD_OK;
 
-    if (!g_r48_table_ready) {
-        k_r48_init_table<<<1, 1, 0, st>>>();
-        CK(cudaGetLastError());
-        g_r48_launches++;
-        g_r48_table_ready = true;
+    {
+        const int r_ = r48_ensure_table(st);
+        if (r_) return r_;
     }
     if (!seeds_dev) {
         dseeds = (uint64_t *)ljmd_dev_alloc(nstreams * 8, st);
@@ -311,11 +330,9 @@ k_mb_apply(float4 *__restrict__ vel, const double *__restrict__ vraw, const doub
 int ljmd_mb_velocities(md_sim *s, double T, uint64_t seed48, double *vraw, double *part, double *mom)
 {
     cudaStream_t st = s->stream;
-    if (!g_r48_table_ready) {
-        k_r48_init_table<<<1, 1, 0, st>>>();
-        CK(cudaGetLastError());
-        g_r48_launches++;
-        g_r48_table_ready = true;
+    {
+        const int r_ = r48_ensure_table(st);
+        if (r_) return r_;
     }
     const int nb = (int)((s->N + MB_T - 1) / MB_T);
     k_mb_draw<<<nb, MB_T, 0, st>>>(s->pos, s->N, seed48, sqrt(T), vraw, part);
@@ -370,11 +387,9 @@ k_kick_andersen(float4 *__restrict__ vel, const float4 *__restrict__ frc, const 
 int ljmd_kick_andersen(md_sim *s)
 {
     cudaStream_t st = s->stream;
-    if (!g_r48_table_ready) {
-        k_r48_init_table<<<1, 1, 0, st>>>();
-        CK(cudaGetLastError());
-        g_r48_launches++;
-        g_r48_table_ready = true;
+    {
+        const int r_ = r48_ensure_table(st);
+        if (r_) return r_;
     }
     const int nb = (int)((s->N + MB_T - 1) / MB_T);
     k_kick_andersen<<<nb, MB_T, 0, st>>>(s->vel, s->frc, s->pos, s->N, s->hdtf, sqrt(s->and_T), s->and_thr, s->and_seed,

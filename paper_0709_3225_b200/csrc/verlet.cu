@@ -32,6 +32,7 @@
 #define VL_MINB 8
 #endif
 #define VL_JMASK 0x7fffffu
+#define VL_CELLMASK 0x3fffffff
 #define VL_INERT (31u << 23)            // offset index 31 = (+side, +side, +side): beyond any cutoff
 
 // offset code of one dimension: 0: same cell, 1: +side, 2: -side, 3: +last, 4: -last
@@ -40,13 +41,22 @@ __device__ __forceinline__ float vl_code_value(int code, const Grid &g)
     return code == 0 ? 0.f : code == 1 ? g.side : code == 2 ? -g.side : code == 3 ? g.last : -g.last;
 }
 
-// cell-local coordinate of the wrapped position x for home cell index c (one dimension)
-__device__ __forceinline__ float vl_local(float x, int c, const Grid &g)
+// cell-local coordinate of the wrapped position x for home cell index c (one dimension).  Exact in every case
+// but one: home cell near the top of the box and the atom wrapped to x ~ 0, where x has bits below the 2^-22
+// grid of l = x + (L - o).  There the stored position is moved onto that grid (by <= 1.2e-7, less than the
+// rounding the drift x + dt v has near the top of the box anyway), so that the local coordinate the force
+// kernels see and the position the caller reads back stay the same point: without it the forces of such an
+// atom are those of a point up to 1.2e-7 away, 2e-5 off on a close pair (measured at N = 2,048,000).
+__device__ __forceinline__ float vl_local(float &x, int c, const Grid &g)
 {
     const float o = (float)c * g.side;                  // exact
     float l = x - o;                                    // exact unless the atom crossed the periodic seam
     if (l > 0.5f * g.L) l = (x - g.L) - o;              // home cell near 0, atom wrapped to the top: x - L is exact
-    else if (l < -0.5f * g.L) l = x + (g.L - o);        // home cell near the top, atom wrapped to x ~ 0
+    else if (l < -0.5f * g.L) {                         // home cell near the top, atom wrapped to x ~ 0
+        const float C = g.L - o;                        // exact
+        l = x + C;
+        x = l - C;                                      // exact, >= 0
+    }
     return l;
 }
 
@@ -57,7 +67,10 @@ __global__ void __launch_bounds__(1) k_vl_decide(VlCtl *ctl, unsigned thr_bits)
     ctl->rebuild = rb;
     ctl->force = 0;
     ctl->maxd2 = 0u;
-    if (rb) ctl->nbuilds++;
+    if (rb) {
+        ctl->nbuilds++;
+        ctl->overflow = 0;                               // every list is rewritten: the build reports afresh
+    }
     ctl->nsteps++;
 }
 
@@ -83,15 +96,15 @@ k_vl_kick_drift(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4
         p.x = wrap_drift(fmaf(dt, v.x, p.x), g.L);
         p.y = wrap_drift(fmaf(dt, v.y, p.y), g.L);
         p.z = wrap_drift(fmaf(dt, v.z, p.z), g.L);
-        pos[i] = p;
         vel[i] = v;
         float4 l = lpos[i];
         const float4 l0 = lbuild[i];
-        const int c = __float_as_int(l.w);
+        const int c = __float_as_int(l.w) & VL_CELLMASK;
         const int cz = c % g.n, cy = (c / g.n) % g.n, cx = c / (g.n * g.n);
         l.x = vl_local(p.x, cx, g);
         l.y = vl_local(p.y, cy, g);
         l.z = vl_local(p.z, cz, g);
+        pos[i] = p;
         lpos[i] = l;
         const float ex = l.x - l0.x, ey = l.y - l0.y, ez = l.z - l0.z;
         d2 = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
@@ -174,7 +187,7 @@ k_vl_build(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, 
     const int i = blockIdx.x * VL_T + threadIdx.x;
     if (i >= N) return;
     const float4 li = lpos[i];
-    const int c = __float_as_int(li.w), n = g.n;
+    const int c = __float_as_int(li.w) & VL_CELLMASK, n = g.n;
     const int cz = c % n, cy = (c / n) % n, cx = c / (n * n);
     int cnt = 0;
     for (int ax = -1; ax <= 1; ax++) {
@@ -207,7 +220,7 @@ k_vl_build(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, 
             }
         }
     }
-    if (cnt > cap) ctl->overflow = 1;
+    if (cnt > cap) atomicMax(&ctl->overflow, cnt);         // the length this list needs
     cnt = min(cnt, cap);
     // pad to a multiple of VL_U with inert entries: the atom itself, displaced by a cell diagonal
     for (; cnt % VL_U; cnt++) list[(size_t)cnt * npad + i] = (unsigned)i | VL_INERT;
@@ -349,6 +362,22 @@ static int vl_alloc(md_sim *s)
     }
     CK(cudaMemsetAsync(s->vl_ctl, 0, sizeof(VlCtl), s->stream));
     (void)g;
+    return MD_OK;
+}
+
+// After an overflow: lists long enough for `need` entries (plus a margin); the next evaluation rebuilds.
+int ljmd_vl_grow(md_sim *s, int need)
+{
+    int cap = need + need / 8 + 8;
+    cap = (cap + 7) / 8 * 8;
+    if (cap <= s->vl_cap) return MD_OK;
+    CK(cudaStreamSynchronize(s->stream));
+    unsigned *nl = (unsigned *)ljmd_dev_alloc((size_t)cap * s->vl_npad * sizeof(unsigned), s->stream);
+    if (!nl) return MD_ENOMEM;
+    ljmd_dev_free(s->vl_list, s->stream);
+    s->vl_list = nl;
+    s->vl_cap = cap;
+    s->layout = LAYOUT_NONE;                             // forces a build at the next evaluation
     return MD_OK;
 }
 

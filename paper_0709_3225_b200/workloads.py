@@ -63,28 +63,17 @@ def fcc_positions(n, rho):
     return pos.astype(np.float32), L
 
 
-def maxwell_boltzmann(uniforms, N, T):
-    """Velocities float32 [N,3] from 6N uniform doubles in [0,1) (Box-Muller, cosine branch).
-
-    For atom i, component c, in order: u1 = uniforms[6i+2c], u2 = uniforms[6i+2c+1];
-    v = sqrt(T) sqrt(-2 ln(1-u1)) cos(2 pi u2).  Then the mean is subtracted and the
-    set rescaled so that sum v^2 = 3 N T (R11), and cast to float32.
-    """
-    u = np.asarray(uniforms, dtype=np.float64).reshape(N, 3, 2)
-    v = np.sqrt(T) * np.sqrt(-2.0 * np.log(1.0 - u[..., 0])) * np.cos(2.0 * np.pi * u[..., 1])
-    v -= v.mean(axis=0, keepdims=True)
-    v *= np.sqrt(3.0 * N * T / np.sum(v * v))
-    return v.astype(np.float32)
-
-
-def md_system(name, uniform_source, seed=MASTER_SEED):
-    """Build a named MD config.  uniform_source(seed48, ndraws) -> float64 array of
-    ndraws uniforms in [0,1) from ONE rand48 stream started at state seed48."""
+def md_system(name, velocity_source, seed=MASTER_SEED):
+    """Build a named MD config.  velocity_source(N, T, seed48) -> float32 [N,3]: Maxwell-Boltzmann
+    velocities at temperature T drawn from ONE rand48 stream started at state seed48 (the recipe of
+    DESIGN.md section 4; the arithmetic lives with the caller: md_init_velocities on the product side,
+    oracle.mb_velocities or the tests' NumPy generator on the test side)."""
     cfg = CONFIGS[name]
     pos, L = fcc_positions(cfg["n"], cfg["rho"])
     N = pos.shape[0]
     x0 = splitmix64(seed) & MASK48
-    vel = maxwell_boltzmann(uniform_source(x0, 6 * N), N, cfg["T"])
+    vel = np.ascontiguousarray(velocity_source(N, cfg["T"], x0), dtype=np.float32)
+    assert vel.shape == (N, 3)
     return dict(name=name, N=N, L=L, pos=pos, vel=vel, rc=RC, eps=EPS, sigma=SIGMA, dt=DT,
                 shifted=SHIFTED, steps=cfg["steps"], algo=cfg["algo"], rho=cfg["rho"], T=cfg["T"])
 

@@ -29,3 +29,20 @@ def oracle_uniforms():
         out, _ = oracle.rand48_fill([seed48], ndraws, kind=2)
         return out[0]
     return src
+
+
+@pytest.fixture(scope="session", autouse=True)
+def torch_side_stream():
+    """GPU tests run with a non-default PyTorch stream current, so that the binding's default plumbing
+    (PyTorch's caching allocator and current stream, north_star: "PyTorch is used only for device memory
+    and streams") is the path every parity test exercises.  No effect without a device."""
+    try:
+        import torch
+    except ImportError:
+        yield
+        return
+    if not torch.cuda.is_available():
+        yield
+        return
+    with torch.cuda.stream(torch.cuda.Stream()):
+        yield

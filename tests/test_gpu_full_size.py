@@ -9,7 +9,7 @@ import numpy as np
 import pytest
 
 import oracle
-from helpers import force_check
+from helpers import check_forces, force_check, maxwell_boltzmann, velocities_from
 from paper_0709_3225_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
@@ -30,50 +30,23 @@ def gpu_uniforms(b):
     return src
 
 
-def near_cutoff_atoms(pos, L, atoms, rc=2.5, tol=4e-7):
-    """Atoms of `atoms` that have a partner with |r^2/rc^2 - 1| < tol (R16), by brute force."""
-    p = pos.astype(np.float64)
-    flagged = set()
-    for i in atoms:
-        d = p - p[i]
-        d -= L * np.rint(d / L)
-        r2 = np.einsum("ij,ij->i", d, d)
-        if np.any(np.abs(r2 / (rc * rc) - 1.0) < tol):
-            flagged.add(int(i))
-    return flagged
-
-
-def check_forces(F, Fo, pos, L):
-    """R15 on every component; violations are accepted only on R16 atoms and only up to the
-    force jump at the cutoff."""
-    F = np.asarray(F, dtype=np.float64)
-    tol = np.maximum(1e-4 * np.abs(Fo), 1e-5)
-    bad = np.argwhere(np.abs(F - Fo) > tol)
-    atoms = sorted(set(int(a) for a in bad[:, 0]))
-    assert len(atoms) <= 200, "too many violations: %d components" % len(bad)
-    flagged = near_cutoff_atoms(pos, L, atoms)
-    for a in atoms:
-        assert a in flagged, ("R15 violated on atom %d without a near-cutoff partner" % a, F[a], Fo[a])
-        assert np.max(np.abs(F[a] - Fo[a])) < 0.04 + 1e-4, (a, F[a], Fo[a])
-    return len(atoms)
-
-
-def run_and_compare(b, name, steps, algo, cross_check=False):
-    sysd = wl.md_system(name, gpu_uniforms(b))
+def run_and_compare(b, name, steps, algo, cross_check=False, shifted=1):
+    sysd = wl.md_system(name, velocities_from(gpu_uniforms(b)))
     N, L = sysd["N"], sysd["L"]
+    assert steps == wl.CONFIGS[name]["steps"]                # the length BASELINE.json names for this config
     import os
     oracle.set_threads(os.cpu_count() or 1)
-    with b.Sim(N, L) as s:
+    with b.Sim(N, L, shifted=shifted) as s:
         s.set_state(sysd["pos"], sysd["vel"])
         s.step(steps, algo)
         ke, pe, w = s.energies()
         F = s.forces()
         p, v = s.get_state()
         assert np.all(p >= 0) and np.all(p < np.float32(L))
-        Fo, peo, wo = oracle.forces(p.astype(np.float64), L, algo=1)
+        Fo, peo, wo = oracle.forces(p.astype(np.float64), L, mode=shifted, algo=1)
         assert np.max(np.abs(Fo)) > 10                       # the state has melted: real forces
         # forces of the last step belong to the returned positions (velocity Verlet is synchronous)
-        nflag = check_forces(F, Fo, p, L)
+        nflag = check_forces(F, Fo, p, L, oracle)
         rel = 1e-9 if algo == 0 else 1e-6                    # DESIGN.md R23
         assert pe == pytest.approx(peo, rel=rel) and w == pytest.approx(wo, rel=rel)
         assert ke == pytest.approx(oracle.kinetic_energy(v.astype(np.float64)), rel=1e-9)
@@ -81,7 +54,7 @@ def run_and_compare(b, name, steps, algo, cross_check=False):
         if cross_check:                                      # R18: the other force path on the same state
             s.set_state(p, v)
             s.compute_forces(1 - algo)
-            nflag += check_forces(s.forces(), Fo, p, L)
+            nflag += check_forces(s.forces(), Fo, p, L, oracle)
             _, pe2, w2 = s.energies()
             assert pe2 == pytest.approx(peo, rel=1e-6) and w2 == pytest.approx(wo, rel=1e-6)
         if algo == 1:
@@ -91,16 +64,45 @@ def run_and_compare(b, name, steps, algo, cross_check=False):
 
 
 def test_c2_allpairs_32000(b):
-    run_and_compare(b, "c2_allpairs_32k", 60, 0, cross_check=True)
+    run_and_compare(b, "c2_allpairs_32k", 1000, 0, cross_check=True)
 
 
 def test_c3_cell_256000_with_allpairs_cross_check(b):
-    run_and_compare(b, "c3_cell_256k", 100, 1, cross_check=True)
+    run_and_compare(b, "c3_cell_256k", 1000, 1, cross_check=True)
+
+
+def test_c3_cell_256000_force_shifted(b):
+    """The paper's own potential (Eq. 3, shifted = 2) at a full size: no cutoff ambiguity there
+    (the force is continuous at rc), so no atom may be excused."""
+    assert run_and_compare(b, "c3_cell_256k", 1000, 1, shifted=2) == 0
 
 
 @pytest.mark.parametrize("name", ["c4a_cell_2048k", "c4b_cell_2048k_rho03"])
 def test_c4_cell_2048000(b, name):
-    run_and_compare(b, name, 40, 1)
+    run_and_compare(b, name, 500, 1)
+
+
+@pytest.mark.parametrize("kernel,fuse", [(1, 0), (3, 0), (2, 1), (3, 1)])
+def test_c3_other_cell_kernels(b, kernel, fuse):
+    """The cell-force kernels that are not the default (the first ballot kernel, the dense kernel, and the
+    integrator fused into the force epilogue) on the full config-3 system, every atom."""
+    sysd = wl.md_system("c3_cell_256k", velocities_from(gpu_uniforms(b)))
+    N, L = sysd["N"], sysd["L"]
+    import os
+    oracle.set_threads(os.cpu_count() or 1)
+    with b.Sim(N, L) as s:
+        s.option("cell_kernel", kernel)
+        s.option("fuse_integrator", fuse)
+        s.set_state(sysd["pos"], sysd["vel"])
+        s.step(300, 1)
+        ke, pe, w = s.energies()
+        F = s.forces()
+        p, v = s.get_state()
+    Fo, peo, wo = oracle.forces(p.astype(np.float64), L, algo=1)
+    assert np.max(np.abs(Fo)) > 10
+    check_forces(F, Fo, p, L, oracle)
+    assert pe == pytest.approx(peo, rel=1e-6) and w == pytest.approx(wo, rel=1e-6)
+    assert ke == pytest.approx(oracle.kinetic_energy(v.astype(np.float64)), rel=1e-9)
 
 
 @pytest.mark.parametrize("name,algo,nsteps", [("c1_allpairs_500", 0, 10000), ("c1_allpairs_500", 1, 10000),
@@ -108,7 +110,7 @@ def test_c4_cell_2048000(b, name):
                                               ("c3_cell_256k", 2, 10000)])
 def test_nve_drift_10k_steps(b, name, algo, nsteps):
     """R17: |<E>_{9000..10000} - <E>_{1000..2000}| / |E(0)| < 1e-4, E sampled every 10 steps."""
-    sysd = wl.md_system(name, gpu_uniforms(b))
+    sysd = wl.md_system(name, velocities_from(gpu_uniforms(b)))
     E = []
     with b.Sim(sysd["N"], sysd["L"]) as s:
         s.set_state(sysd["pos"], sysd["vel"])

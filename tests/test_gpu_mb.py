@@ -5,6 +5,7 @@ import pytest
 
 import oracle
 from conftest import golden_lines
+from helpers import maxwell_boltzmann, velocities_from
 from paper_0709_3225_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
@@ -59,7 +60,7 @@ def test_config1_pin_and_errors(b):
 @pytest.mark.parametrize("algo", [0, 1, 2])
 def test_andersen_thermostat_matches_the_oracle(b, algo, oracle_uniforms):
     """30 steps with collisions (nu dt = 0.05) on config 1 against the oracle's step + andersen_collide."""
-    c1 = wl.md_system("c1_allpairs_500", oracle_uniforms)
+    c1 = wl.md_system("c1_allpairs_500", velocities_from(oracle_uniforms))
     N, L, T, nu, seed = c1["N"], c1["L"], 1.5, 10.0, 0x0123456789AB
     with b.Sim(N, L) as s:
         s.option("andersen_T", T)
@@ -88,7 +89,7 @@ def test_andersen_thermostat_matches_the_oracle(b, algo, oracle_uniforms):
 
 
 def test_andersen_off_is_plain_nve(b, oracle_uniforms):
-    c1 = wl.md_system("c1_allpairs_500", oracle_uniforms)
+    c1 = wl.md_system("c1_allpairs_500", velocities_from(oracle_uniforms))
     out = []
     for nu in (None, 0.0):
         with b.Sim(c1["N"], c1["L"]) as s:

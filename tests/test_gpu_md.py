@@ -4,7 +4,7 @@ import numpy as np
 import pytest
 
 import oracle
-from helpers import force_check, melt
+from helpers import force_check, maxwell_boltzmann, melt, velocities_from
 from paper_0709_3225_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
@@ -135,7 +135,7 @@ def test_allpairs_tiled_after_drift_without_resort(b, oracle_uniforms):
     """Between re-sorts atoms leave their tile (and cross the periodic seam): the per-block
     bounding box check must keep the result exact."""
     pos, L = wl.fcc_positions(10, 0.8)
-    vel = wl.maxwell_boltzmann(oracle_uniforms(wl.splitmix64(5) & wl.MASK48, 6 * 4000), 4000, 2.0)
+    vel = maxwell_boltzmann(oracle_uniforms(wl.splitmix64(5) & wl.MASK48, 6 * 4000), 4000, 2.0)
     with b.Sim(4000, L) as s:
         s.option("ap_R", 2)
         s.option("sort_every", 1000)
@@ -218,7 +218,7 @@ def test_error_codes(b):
 
 @pytest.fixture(scope="module")
 def c1(oracle_uniforms):
-    return wl.md_system("c1_allpairs_500", oracle_uniforms)
+    return wl.md_system("c1_allpairs_500", velocities_from(oracle_uniforms))
 
 
 @pytest.mark.parametrize("algo", [0, 1])
@@ -276,7 +276,7 @@ def test_melted_snapshot_n4000(b, oracle_uniforms):
     """Forces on a melted N = 4000 snapshot (pair forces up to ~70), both algos."""
     pos, L = wl.fcc_positions(10, 0.8)
     x0 = wl.splitmix64(77) & wl.MASK48
-    vel = wl.maxwell_boltzmann(oracle_uniforms(x0, 6 * 4000), 4000, 1.0)
+    vel = maxwell_boltzmann(oracle_uniforms(x0, 6 * 4000), 4000, 1.0)
     with b.Sim(4000, L) as s:
         s.set_state(pos, vel)
         s.step(400, b.MD_CELL)

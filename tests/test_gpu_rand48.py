@@ -74,9 +74,12 @@ def test_single_stream_skip_ahead_2p24(b):
     assert int(st[0]) == oracle.rand48_skip(x0, n)
 
 
-def test_config5_sampled_full_size(b):
-    """BASELINE config 5 at full size on device buffers; sampled streams and windows are
-    compared with the sequential oracle, final states with its skip-ahead."""
+def test_config5_full_size_every_element(b):
+    """BASELINE config 5 at full size on device buffers, every element of every stream against the
+    sequential oracle (memcmp; "the first N random numbers of the lrand48
+    series"), as uint32 and as double: 65,536 streams x 4,096 draws in chunks of 8,192 streams, then the
+    single stream of 2^28 draws in chunks of 2^24 with the oracle's state carried from chunk to chunk
+    (no skip-ahead on the oracle's side).  Returned states included."""
     import torch
     ns, nd = wl.C5_NSTREAMS, wl.C5_NDRAWS
     seeds = wl.stream_seeds(wl.MASTER_SEED, ns)
@@ -84,21 +87,25 @@ def test_config5_sampled_full_size(b):
         dseeds = torch.from_numpy(seeds.astype(np.int64)).cuda()
         out = torch.empty(ns * nd, dtype=tdt, device="cuda")
         b.rand48_fill(dseeds.data_ptr(), ns, nd, kind, out.data_ptr())
-        pick = [0, 1, 777, 32768, ns - 1]
-        ref, rs = oracle.rand48_fill(seeds[pick], nd, kind)
-        got = out.view(ns, nd)[pick].cpu().numpy()
-        assert np.array_equal(got.view(np.uint8), ref.view(np.uint8))
         st = dseeds.cpu().numpy().view(np.uint64)
-        assert np.array_equal(st[pick], rs)
-        assert all(int(st[i]) == oracle.rand48_skip(int(seeds[i]), nd) for i in range(0, ns, 997))
-    # single stream of 2^28 draws: windows around segment boundaries + the tail
+        rows = out.view(ns, nd)
+        for lo in range(0, ns, 8192):
+            ref, rs = oracle.rand48_fill(seeds[lo:lo + 8192], nd, kind)
+            got = rows[lo:lo + 8192].cpu().numpy()
+            assert np.array_equal(got.view(np.uint8), ref.view(np.uint8)), (kind, lo)
+            assert np.array_equal(st[lo:lo + 8192], rs), (kind, lo)
+        del out, rows
     n = wl.C5_SINGLE_NDRAWS
     x0 = int(seeds[0])
-    d1 = torch.tensor([x0], dtype=torch.int64, device="cuda")
-    out = torch.empty(n, dtype=torch.int32, device="cuda")
-    b.rand48_fill(d1.data_ptr(), 1, n, 0, out.data_ptr())
-    for start in (0, 2047, 2048, 4096 * 1000 - 3, n // 2 - 100, n - 5000):
-        cnt = min(5000, n - start)
-        ref, _ = oracle.rand48_fill([oracle.rand48_skip(x0, start)], cnt, 0)
-        assert np.array_equal(out[start:start + cnt].cpu().numpy().view(np.uint32), ref[0]), start
-    assert int(d1.cpu().numpy().view(np.uint64)[0]) == oracle.rand48_skip(x0, n)
+    for kind, tdt in ((0, torch.int32), (2, torch.float64)):
+        d1 = torch.tensor([x0], dtype=torch.int64, device="cuda")
+        out = torch.empty(n, dtype=tdt, device="cuda")
+        b.rand48_fill(d1.data_ptr(), 1, n, kind, out.data_ptr())
+        state, chunk = x0, 1 << 24
+        for lo in range(0, n, chunk):
+            ref, rs = oracle.rand48_fill([state], chunk, kind)
+            got = out[lo:lo + chunk].cpu().numpy()
+            assert np.array_equal(got.view(np.uint8), ref[0].view(np.uint8)), (kind, lo)
+            state = int(rs[0])
+        assert int(d1.cpu().numpy().view(np.uint64)[0]) == state == oracle.rand48_skip(x0, n)
+        del out

@@ -198,3 +198,20 @@ def test_near_cutoff_pairs():
     pos = np.array([[1.0, 1.0, 1.0], [3.5 - 1e-7, 1.0, 1.0], [1.0, 3.0, 1.0]])
     pairs, n = oracle.near_cutoff_pairs(pos, 12.0, tol=4e-7)
     assert n == 2 and sorted(map(tuple, pairs)) == [(0, 1), (1, 0)]
+
+
+def test_near_cutoff_pairs_cell_lists_the_same_pairs():
+    """The linked-cell lister against the O(N^2) one: a fluid-like system with a wide window (so that the
+    lists are long), a pair planted across the periodic seam exactly in the window, and the 3-cell box."""
+    rng = np.random.default_rng(5)
+    for L, N, tol in ((12.0, 900, 2e-3), (7.6, 300, 5e-3)):
+        pos = rng.random((N, 3)) * L
+        pos[0] = (0.05, 3.0, 3.0)
+        pos[1] = (L - 2.45 + 1e-7, 3.0, 3.0)             # r = 2.5 - 1e-7 through the seam
+        a, na = oracle.near_cutoff_pairs(pos, L, tol=tol)
+        c, nc = oracle.near_cutoff_pairs_cell(pos, L, tol=tol)
+        assert na == nc and na > 20
+        assert sorted(map(tuple, a)) == sorted(map(tuple, c))
+        assert (0, 1) in set(map(tuple, c)) and (1, 0) in set(map(tuple, c))
+    with pytest.raises(ValueError):
+        oracle.near_cutoff_pairs_cell(rng.random((10, 3)) * 6.0, 6.0)

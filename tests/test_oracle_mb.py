@@ -1,11 +1,12 @@
 """Pins of the oracle's Maxwell-Boltzmann generator (oracle.mb_velocities): the printed values of the
 survey's independent NumPy probe (tests/golden/config1_trajectory.txt), the harness generator
-(workloads.maxwell_boltzmann fed with the oracle's sequential rand48), and the defining moments."""
+(helpers.maxwell_boltzmann, the harness generator, fed with the oracle's sequential rand48), and the defining moments."""
 import numpy as np
 import pytest
 
 import oracle
 from conftest import golden_lines
+from helpers import maxwell_boltzmann, velocities_from
 from paper_0709_3225_b200 import workloads as wl
 
 
@@ -29,7 +30,7 @@ def test_config1_values_of_the_survey_probe(g):
 def test_matches_the_harness_generator_and_the_moments(N, T, seed, oracle_uniforms):
     x0 = wl.splitmix64(seed) & wl.MASK48
     v, _ = oracle.mb_velocities(N, T, x0)
-    ref = wl.maxwell_boltzmann(oracle_uniforms(x0, 6 * N), N, T)        # float32
+    ref = maxwell_boltzmann(oracle_uniforms(x0, 6 * N), N, T)        # float32
     assert np.max(np.abs(v - ref.astype(np.float64))) < 3e-7             # FP32 cast of the same numbers
     assert np.max(np.abs(v.sum(axis=0))) < 1e-10 * N                      # zero net momentum
     assert np.sum(v * v) == pytest.approx(3.0 * N * T, rel=1e-13)         # R11

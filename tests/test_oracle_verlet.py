@@ -5,6 +5,7 @@ import pytest
 
 import oracle
 from conftest import golden_lines
+from helpers import maxwell_boltzmann, velocities_from
 from paper_0709_3225_b200 import workloads as wl
 
 
@@ -14,7 +15,7 @@ def golden_c1():
 
 @pytest.fixture(scope="module")
 def c1(oracle_uniforms):
-    return wl.md_system("c1_allpairs_500", oracle_uniforms)
+    return wl.md_system("c1_allpairs_500", velocities_from(oracle_uniforms))
 
 
 def test_free_flight_closed_form():
