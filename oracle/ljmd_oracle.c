@@ -158,10 +158,14 @@ int forces_cell(int64_t N, const double *pos, double L, double rc,
         next[i] = head[id];
         head[id] = i;
     }
-    double pe = 0.0, w = 0.0;
-#pragma omp parallel for reduction(+ : pe, w) schedule(static)
+    /* per-atom halves of U and W, summed in atom order after the loop: the result does not
+     * depend on the number of threads */
+    double *pei = (double *)malloc((size_t)N * sizeof(double));
+    double *wi = (double *)malloc((size_t)N * sizeof(double));
+#pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < N; i++) {
         double fi[3] = {0.0, 0.0, 0.0};
+        double pe = 0.0, w = 0.0;
         for (int ax = -1; ax <= 1; ax++)
         for (int ay = -1; ay <= 1; ay++)
         for (int az = -1; az <= 1; az++) {
@@ -188,9 +192,18 @@ int forces_cell(int64_t N, const double *pos, double L, double rc,
         }
         for (int c = 0; c < 3; c++)
             F[3 * i + c] = fi[c];
+        pei[i] = pe;
+        wi[i] = w;
+    }
+    double pe = 0.0, w = 0.0;
+    for (int64_t i = 0; i < N; i++) {
+        pe += pei[i];
+        w += wi[i];
     }
     *PE = pe;
     *W = w;
+    free(pei);
+    free(wi);
     free(head);
     free(next);
     free(cxyz);
