@@ -46,6 +46,10 @@ def lib():
         L.forces_cell.restype = i32
         L.cell_grid.argtypes = [d, d, ctypes.POINTER(i32), pd]
         L.cell_grid.restype = i32
+        L.yukawa_pair.argtypes = [ctypes.c_int, d, d, d, d, ctypes.POINTER(d), ctypes.POINTER(d)]
+        L.yukawa_pair.restype = ctypes.c_int
+        L.set_potential.argtypes = [ctypes.c_int, d, d]
+        L.set_potential.restype = None
         L.near_cutoff_pairs.argtypes = [i64, vp, d, d, d, vp, i64]
         L.near_cutoff_pairs.restype = i64
         L.near_cutoff_pairs_cell.argtypes = [i64, vp, d, d, d, vp, i64]
@@ -98,6 +102,29 @@ def lj_pair(mode, r2, eps=1.0, sigma=1.0, rc=2.5):
     u, fr = ctypes.c_double(), ctypes.c_double()
     inside = lib().lj_pair(mode, r2, eps, sigma, rc, ctypes.byref(u), ctypes.byref(fr))
     return bool(inside), u.value, fr.value
+
+
+def yukawa_pair(mode, r2, A=1.0, kappa=1.0, rc=2.5):
+    """(inside, U, f/r) of the screened Coulomb pair U = A exp(-kappa r)/r.  PAPER.md:184 (other pair
+    potentials, "including the coulombic interaction"); SURVEY 8(f) item 4."""
+    u, fr = ctypes.c_double(), ctypes.c_double()
+    inside = lib().yukawa_pair(mode, r2, A, kappa, rc, ctypes.byref(u), ctypes.byref(fr))
+    return bool(inside), u.value, fr.value
+
+
+class potential:
+    """with oracle.potential(1, A, kappa): ... -- the force loops (and verlet_*) evaluate the Yukawa pair inside
+    the block, Lennard-Jones again after it."""
+
+    def __init__(self, kind, A=1.0, kappa=1.0):
+        self.args = (int(kind), float(A), float(kappa))
+
+    def __enter__(self):
+        lib().set_potential(*self.args)
+        return self
+
+    def __exit__(self, *a):
+        lib().set_potential(0, 1.0, 1.0)
 
 
 def forces(pos, L, rc=2.5, eps=1.0, sigma=1.0, mode=1, algo=0):

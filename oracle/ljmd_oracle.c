@@ -15,6 +15,8 @@
  *
  * Pins (tests/test_oracle_*.py, run with -m "not gpu"):
  *   lj_pair            closed forms, constants at rc = 2.5, finite differences
+ *   yukawa_pair        Coulomb limit kappa = 0 by hand, U at r = 1/kappa, finite differences,
+ *                      two-charge force by hand, shift modes vanish at rc
  *   forces_allpairs    fcc shell sums, dimer/trimer by hand, sum F = 0,
  *                      translation invariance, scale invariance
  *   forces_cell        agreement with forces_allpairs, paper's L = 11 example
@@ -79,6 +81,70 @@ int lj_pair(int mode, double r2, double eps, double sigma, double rc,
     return 1;
 }
 
+/* ----------------------------------------------------------------- O1b --
+ * A second pair potential through the same loops (PAPER.md:184,
+ * Outlook: "it is trivial to replace this potential by other pair-potentials, including
+ * the coulombic interaction"): the screened Coulomb (Yukawa) interaction between equal
+ * charges,
+ *     U_Y(r) = A exp(-kappa r) / r,
+ *     f_Y(r) = -dU_Y/dr = A exp(-kappa r) (1/r^2 + kappa/r),
+ * which is the bare Coulomb pair A/r for kappa = 0.  Truncated at rc with the same three
+ * shift modes as lj_pair (the paper treats no long-range part: PAPER.md:184-188 leaves
+ * Ewald-type sums to future work).  Outputs as lj_pair.
+ */
+static double u_yukawa(double r, double A, double kappa)
+{
+    return A * exp(-kappa * r) / r;
+}
+
+static double f_yukawa(double r, double A, double kappa)
+{
+    return A * exp(-kappa * r) * (1.0 / (r * r) + kappa / r);
+}
+
+int yukawa_pair(int mode, double r2, double A, double kappa, double rc,
+                double *U, double *f_over_r)
+{
+    if (!(r2 < rc * rc)) {
+        *U = 0.0;
+        *f_over_r = 0.0;
+        return 0;
+    }
+    double r = sqrt(r2);
+    double u = u_yukawa(r, A, kappa);
+    double f = f_yukawa(r, A, kappa);
+    if (mode == 1) {
+        u -= u_yukawa(rc, A, kappa);
+    } else if (mode == 2) {
+        double f_rc = f_yukawa(rc, A, kappa);
+        u = u - u_yukawa(rc, A, kappa) + (r - rc) * f_rc;
+        f -= f_rc;
+    }
+    *U = u;
+    *f_over_r = f / r;
+    return 1;
+}
+
+/* Which pair potential the force loops below evaluate: 0 = Lennard-Jones (eps, sigma from
+ * the call), 1 = Yukawa (A, kappa set here).  Test-harness state, default 0. */
+static int g_pot_kind = 0;
+static double g_pot_A = 1.0, g_pot_kappa = 1.0;
+
+void set_potential(int kind, double A, double kappa)
+{
+    g_pot_kind = kind;
+    g_pot_A = A;
+    g_pot_kappa = kappa;
+}
+
+static int pair_term(int mode, double r2, double eps, double sigma, double rc,
+                     double *U, double *f_over_r)
+{
+    if (g_pot_kind == 1)
+        return yukawa_pair(mode, r2, g_pot_A, g_pot_kappa, rc, U, f_over_r);
+    return lj_pair(mode, r2, eps, sigma, rc, U, f_over_r);
+}
+
 /* ------------------------------------------------------------------ O2 --
  * All-pairs force, PAPER.md:49-52 (Eq. 1):
  *     F_i = - sum_{j != i} f(|r_j - r_i|) (r_j - r_i)/|r_j - r_i|
@@ -102,7 +168,7 @@ void forces_allpairs(int64_t N, const double *pos, double L, double rc,
                 r2 += d[c] * d[c];
             }
             double u, fr;
-            if (lj_pair(mode, r2, eps, sigma, rc, &u, &fr)) {
+            if (pair_term(mode, r2, eps, sigma, rc, &u, &fr)) {
                 for (int c = 0; c < 3; c++) {
                     F[3 * i + c] -= fr * d[c];
                     F[3 * j + c] += fr * d[c];
@@ -182,7 +248,7 @@ int forces_cell(int64_t N, const double *pos, double L, double rc,
                     r2 += d[c] * d[c];
                 }
                 double u, fr;
-                if (lj_pair(mode, r2, eps, sigma, rc, &u, &fr)) {
+                if (pair_term(mode, r2, eps, sigma, rc, &u, &fr)) {
                     for (int c = 0; c < 3; c++)
                         fi[c] -= fr * d[c];
                     pe += 0.5 * u;

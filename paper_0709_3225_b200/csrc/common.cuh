@@ -136,6 +136,7 @@ struct md_sim {
     bool precise_r2_user;         // "precise_r2" was set through md_set_option
     int cell_group;               // cells per row group of the cell-force kernel; 0 = automatic
     int cell_kernel;              // 2 (default): force_cell2.cu; 3: force_cell3.cu (dense); 1: force_cell.cu
+    bool cell_skin_on;            // option "cell_skin" > 0: MD_CELL runs on skin cells (verlet.cu)
     bool fuse_integrator;         // option "fuse_integrator": interior steps integrate in the force kernel's epilogue
     int64_t launches, steps_done;
     // CUDA graphs of one "unit" of interior steps (ljmd_api.cu): the unit is the number of steps after
@@ -153,7 +154,7 @@ struct md_sim {
     int64_t n_phase[TAG_COUNT];
 };
 
-enum { LAYOUT_NONE = 0, LAYOUT_CELL = 1, LAYOUT_TILE = 2, LAYOUT_VERLET = 3 };
+enum { LAYOUT_NONE = 0, LAYOUT_CELL = 1, LAYOUT_TILE = 2, LAYOUT_VERLET = 3, LAYOUT_SKINCELL = 4 };
 // Record an event; the time since the previous tick is attributed to `tag`.
 void ljmd_tick(md_sim *s, int tag);
 int ljmd_collect_ticks(md_sim *s);
@@ -179,6 +180,8 @@ int ljmd_vl_stats(md_sim *s, int *nbuilds, int *nsteps, int *overflow);
 int ljmd_vl_grow(md_sim *s, int need);               // longer lists after an overflow; the next evaluation rebuilds
 int ljmd_cell_build(md_sim *s);
 int ljmd_forces_cell(md_sim *s);
+int ljmd_forces_cell2_on(md_sim *s, const Grid &g, double stray, bool energy, bool fused);   // the same on any grid whose lpos/cell_start are current
+int ljmd_forces_skincell(md_sim *s, bool energy);    // verlet.cu: cells of side >= rc + skin, re-sorted when the skin is used up
 int ljmd_forces_cell2(md_sim *s, bool energy, bool fused);   // force_cell2.cu; energy = false: forces only; fused: the epilogue integrates
 int ljmd_forces_cell3(md_sim *s, bool energy, bool fused);   // force_cell3.cu; fused: the epilogue integrates
 int ljmd_kick_drift_bin3(md_sim *s, int kicks);      // cells.cu: lean build (rank in vel.w)

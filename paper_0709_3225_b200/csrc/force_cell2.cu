@@ -563,12 +563,12 @@ int ljmd_fc2_group_cells(const md_sim *s, const Grid &g)
 }
 
 template <int KK>
-static void fc2_launch(md_sim *s, const dim3 grid, const F2Const &K, double *ppe, double *pw, bool energy, bool fused)
+static void fc2_launch(md_sim *s, const Grid &g, const dim3 grid, const F2Const &K, double *ppe, double *pw, bool energy, bool fused)
 {
     const PairParams &P = s->pp;
     const int nmax = (int)s->N - 1;
 #define F2_LAUNCH(M2, EN, FU) \
-    k_fc2<KK, M2, EN, FU><<<grid, 32, 0, s->stream>>>(s->lpos, s->cell_start, s->grid, P, K, s->frc, ppe, pw, nmax, s->pos, s->vel, s->pos2, s->cell_count)
+    k_fc2<KK, M2, EN, FU><<<grid, 32, 0, s->stream>>>(s->lpos, s->cell_start, g, P, K, s->frc, ppe, pw, nmax, s->pos, s->vel, s->pos2, s->cell_count)
     if (fused) {                                    // interior steps: forces only
         if (P.mode == 2) F2_LAUNCH(true, false, true); else F2_LAUNCH(false, false, true);
     } else if (P.mode == 2) {
@@ -582,8 +582,14 @@ static void fc2_launch(md_sim *s, const dim3 grid, const F2Const &K, double *ppe
 // energy = false: forces only (interior steps of md_step, whose PE and virial nobody can read)
 int ljmd_forces_cell2(md_sim *s, bool energy, bool fused)
 {
+    return ljmd_forces_cell2_on(s, s->grid, 0.0, energy, fused);
+}
+
+// The same kernel on any cell grid whose lpos/cell_start are current.  `stray`: how far an atom may sit outside
+// its cell (skin cells between rebuilds, verlet.cu: half the skin); it widens the filter's rounding margin.
+int ljmd_forces_cell2_on(md_sim *s, const Grid &g, double stray, bool energy, bool fused)
+{
     if (fused) energy = false;
-    const Grid &g = s->grid;
     const int kz = ljmd_fc2_group_cells(s, g);
     const int nzu = (g.n + kz - 1) / kz;
     const dim3 grid(nzu, g.n, g.n);
@@ -600,14 +606,14 @@ int ljmd_forces_cell2(md_sim *s, bool energy, bool fused)
     // offset to FP32 rounding; the FP64 window is widened to r^2 < 1.5 sigma^2 so that every pair
     // with |df/dr| > 5 is still evaluated from the exact coordinates.
     double p2 = P.precise_r2;
-    if (kz > 1 && !s->precise_r2_user) p2 = fmax(p2, 1.5 * P.sig2);
+    if ((kz > 1 || stray > 0.0) && !s->precise_r2_user) p2 = fmax(p2, 1.5 * P.sig2);
     K.p2 = (float)fmin(p2, 3.0e38);
     K.h = 0.5f * g.side;
     K.hd = (double)K.h;
     K.nzu = nzu;
-    K.tile_exact = (kz == 1 && 1.5 * (double)g.last < 4.0 && (double)g.side >= 2.0) ? 1 : 0;
+    K.tile_exact = (kz == 1 && stray == 0.0 && 1.5 * (double)g.last < 4.0 && (double)g.side >= 2.0) ? 1 : 0;
     // farthest staged candidate from the frame centre, per dimension; FP32 rounding of the expanded form
-    const double reach_xy = 1.5 * (double)g.last, reach_z = (0.5 * kz + 1.0) * (double)g.last;
+    const double reach_xy = 1.5 * (double)g.last + stray, reach_z = (0.5 * kz + 1.0) * (double)g.last + stray;
     K.rc2_thr = (float)(P.rc2 * (1.0 + 4e-6) + 4.0e-6 * (2.0 * reach_xy * reach_xy + reach_z * reach_z) + 1e-6 * P.rc2);
     K.sig2 = P.sig2f;
     K.eps24 = P.eps24f;
@@ -617,10 +623,10 @@ int ljmd_forces_cell2(md_sim *s, bool energy, bool fused)
     K.hdt = s->hdtf;
     K.dt = s->dtf;
     switch (kz) {
-    case 1: fc2_launch<1>(s, grid, K, ppe, pw, energy, fused); break;
-    case 2: fc2_launch<2>(s, grid, K, ppe, pw, energy, fused); break;
-    case 3: fc2_launch<3>(s, grid, K, ppe, pw, energy, fused); break;
-    default: fc2_launch<5>(s, grid, K, ppe, pw, energy, fused); break;
+    case 1: fc2_launch<1>(s, g, grid, K, ppe, pw, energy, fused); break;
+    case 2: fc2_launch<2>(s, g, grid, K, ppe, pw, energy, fused); break;
+    case 3: fc2_launch<3>(s, g, grid, K, ppe, pw, energy, fused); break;
+    default: fc2_launch<5>(s, g, grid, K, ppe, pw, energy, fused); break;
     }
     CKL(s);
     ljmd_tick(s, TAG_FORCE);

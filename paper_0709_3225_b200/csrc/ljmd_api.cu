@@ -441,6 +441,7 @@ static int check_algo(md_sim *s, int algo)
 {
     if (algo != MD_ALLPAIRS && algo != MD_CELL && algo != MD_VERLET) return MD_EINVAL;
     if (algo == MD_CELL && (s->grid_paper_n < 3 || s->grid.n < 3)) return MD_EDOMAIN;
+    if (algo == MD_CELL && s->cell_skin_on && s->vgrid.n < 3) return MD_EDOMAIN;
     if (algo == MD_VERLET && s->vgrid.n < 3) return MD_EDOMAIN;
     return MD_OK;
 }
@@ -453,6 +454,8 @@ static int eval_forces(md_sim *s, int algo, bool energy = true, bool fuse = fals
     int r;
     if (algo == MD_VERLET) {
         if ((r = ljmd_forces_verlet(s))) return r;
+    } else if (algo == MD_CELL && s->cell_skin_on) {
+        if ((r = ljmd_forces_skincell(s, energy))) return r;
     } else if (algo == MD_CELL && s->cell_kernel >= 2) {
         if ((r = ljmd_cell_build3(s))) return r;
         ljmd_tick(s, TAG_BUILD);
@@ -474,9 +477,11 @@ static int eval_forces(md_sim *s, int algo, bool energy = true, bool fuse = fals
 static int one_step(md_sim *s, int algo, int kicks, bool last, bool energy, bool may_fuse = true)
 {
     int r;
-    const bool k3 = algo == MD_CELL && s->cell_kernel >= 2;      // lean build, fusable force kernel
+    const bool skinc = algo == MD_CELL && s->cell_skin_on;        // slots are stable between re-sorts: the list path's integrator
+    const bool k3 = algo == MD_CELL && s->cell_kernel >= 2 && !skinc;      // lean build, fusable force kernel
     if (!(k3 && s->fused_pending)) {                   // else: the previous force kernel has integrated already
-        if ((r = (algo == MD_CELL) ? (k3 ? ljmd_kick_drift_bin3(s, kicks) : ljmd_kick_drift_bin(s, kicks))
+        if ((r = skinc ? ljmd_vl_kick_drift(s, kicks)
+                 : (algo == MD_CELL) ? (k3 ? ljmd_kick_drift_bin3(s, kicks) : ljmd_kick_drift_bin(s, kicks))
                                    : (algo == MD_VERLET) ? ljmd_vl_kick_drift(s, kicks) : ljmd_kick_drift(s, kicks)))
             return r;
         ljmd_tick(s, TAG_INTEGRATE);
@@ -493,6 +498,7 @@ static int one_step(md_sim *s, int algo, int kicks, bool last, bool energy, bool
 // every step; the all-pairs path re-sorts (and swaps) every sort_every steps.
 static int graph_unit(const md_sim *s, int algo)
 {
+    if (algo == MD_CELL && s->cell_skin_on) return 1;
     if (algo == MD_CELL) return 2;
     if (algo == MD_VERLET) return 1;                  // no buffer swaps: builds are decided and done on the device
     if (s->ap_tiled && !s->ap_force_general) return 2 * s->sort_every;
@@ -618,7 +624,8 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
     if (r) return r;
     // the neighbour-list integrator needs the lists' local coordinates: evaluate first if another
     // path (or md_set_state) ran last
-    if (!s->forces_valid || (algo == MD_VERLET && s->layout != LAYOUT_VERLET && nsteps > 0)) {
+    if (!s->forces_valid || (algo == MD_VERLET && s->layout != LAYOUT_VERLET && nsteps > 0) ||
+        (algo == MD_CELL && s->cell_skin_on && s->layout != LAYOUT_SKINCELL && nsteps > 0)) {
         if ((r = eval_forces_checked(s, algo))) return r;
         if ((r = ljmd_ke_only(s))) return r;
         s->forces_valid = true;
@@ -715,9 +722,20 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
     } else if (!strcmp(key, "vl_naive_build")) {
         s->vl_naive_build = value != 0.0;
     } else if (!strcmp(key, "skin")) {
-        if (!(value > 0) || s->vl_list) return MD_EINVAL;          // before the first use of MD_VERLET
+        if (!(value > 0) || s->vl_ctl) return MD_EINVAL;           // before the first use of MD_VERLET / skin cells
         s->skin = value;
         setup_grid(s);
+    } else if (!strcmp(key, "cell_skin")) {
+        // MD_CELL on cells of side >= rc + value, re-sorted only when an atom has strayed value / 2 (0 = off:
+        // the cell list is rebuilt every step).  Shares the skin with MD_VERLET: set before either is used.
+        if (!(value >= 0) || !isfinite(value)) return MD_EINVAL;
+        if (value > 0 && value != s->skin) {
+            if (s->vl_ctl) return MD_EINVAL;
+            s->skin = value;
+            setup_grid(s);
+        }
+        s->cell_skin_on = value > 0;
+        s->layout = LAYOUT_NONE;
     } else if (!strcmp(key, "cell_group")) {
         if (value < 0 || value > 5) return MD_EINVAL;
         s->cell_group = (int)value;

@@ -339,9 +339,26 @@ k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams 
 
 // ---------------------------------------------------------------------------------------
 // Host side.
+// Control block and build-time coordinates: shared by the neighbour-list path and the skin-cell path.
+static int vl_alloc_base(md_sim *s)
+{
+    if (s->vl_ctl) return MD_OK;
+    s->vl_lbuild = (float4 *)ljmd_dev_alloc((size_t)s->N * sizeof(float4), s->stream);
+    s->vl_ctl = (VlCtl *)ljmd_dev_alloc(sizeof(VlCtl), s->stream);
+    if (!s->vl_lbuild || !s->vl_ctl) {
+        ljmd_dev_free(s->vl_lbuild, s->stream); ljmd_dev_free(s->vl_ctl, s->stream);
+        s->vl_lbuild = nullptr; s->vl_ctl = nullptr;
+        return MD_ENOMEM;
+    }
+    CK(cudaMemsetAsync(s->vl_ctl, 0, sizeof(VlCtl), s->stream));
+    return MD_OK;
+}
+
 static int vl_alloc(md_sim *s)
 {
     if (s->vl_list) return MD_OK;
+    int r0 = vl_alloc_base(s);
+    if (r0) return r0;
     const Grid &g = s->vgrid;
     if (s->N > (int64_t)VL_JMASK) return MD_EUNSUPPORTED;               // slot index must fit 23 bits
     const double rl = s->rc + s->skin;
@@ -352,15 +369,11 @@ static int vl_alloc(md_sim *s)
     s->vl_npad = (int)((s->N + 31) / 32 * 32);
     s->vl_list = (unsigned *)ljmd_dev_alloc((size_t)cap * s->vl_npad * sizeof(unsigned), s->stream);
     s->vl_count = (int *)ljmd_dev_alloc((size_t)s->N * sizeof(int), s->stream);
-    s->vl_lbuild = (float4 *)ljmd_dev_alloc((size_t)s->N * sizeof(float4), s->stream);
-    s->vl_ctl = (VlCtl *)ljmd_dev_alloc(sizeof(VlCtl), s->stream);
-    if (!s->vl_list || !s->vl_count || !s->vl_lbuild || !s->vl_ctl) {
+    if (!s->vl_list || !s->vl_count) {
         ljmd_dev_free(s->vl_list, s->stream); ljmd_dev_free(s->vl_count, s->stream);
-        ljmd_dev_free(s->vl_lbuild, s->stream); ljmd_dev_free(s->vl_ctl, s->stream);
-        s->vl_list = nullptr; s->vl_count = nullptr; s->vl_lbuild = nullptr; s->vl_ctl = nullptr;
+        s->vl_list = nullptr; s->vl_count = nullptr;
         return MD_ENOMEM;
     }
-    CK(cudaMemsetAsync(s->vl_ctl, 0, sizeof(VlCtl), s->stream));
     (void)g;
     return MD_OK;
 }
@@ -403,17 +416,17 @@ int ljmd_vl_kick_drift(md_sim *s, int kicks)
     return MD_OK;
 }
 
-// Decide, (re)build if the device-side flag says so, evaluate forces from the lists.
-int ljmd_forces_verlet(md_sim *s)
+// Decide on the device whether the skin has been used up, and if so re-sort the atoms into the cells of
+// s->vgrid (histogram, scan, scatter, copy back: every kernel returns at once when the flag is clear).
+static int vl_decide_and_sort(md_sim *s, int layout)
 {
-    int r = vl_alloc(s);
-    if (r) return r;
-    const int N = (int)s->N, nbl = (N + VL_T - 1) / VL_T;
+    int r;
+    const int N = (int)s->N;
     const int nb = min((N + 255) / 256, 148 * 16);            // grid-stride kernels: idle launches stay cheap
     const Grid &g = s->vgrid;
-    if (s->layout != LAYOUT_VERLET) {
+    if (s->layout != layout) {
         if ((r = vl_force_build(s))) return r;
-        s->layout = LAYOUT_VERLET;
+        s->layout = layout;
     }
     const float half = 0.5f * (float)s->skin;
     float thr = half * half;
@@ -429,6 +442,32 @@ int ljmd_forces_verlet(md_sim *s)
     CKL(s);
     k_vl_copyback<<<nb, 256, 0, s->stream>>>(s->pos, s->vel, s->vl_lbuild, s->pos2, s->vel2, s->lpos, N, s->vl_ctl);
     CKL(s);
+    return MD_OK;
+}
+
+// Skin cells ("use an even larger skin and therefore update the cell lists
+// only every couple of time steps"): cells of side >= rc + skin; between rebuilds every atom keeps its slot
+// and home cell, the integrator keeps its local coordinate in that cell's frame (k_vl_kick_drift), and the
+// cell-force kernel runs on those cells with the exact cutoff rc.  An atom strays at most skin / 2 from where
+// it was at the last rebuild before the device-side decision re-sorts, so no pair inside rc is ever outside the
+// 27 home cells.  Same forces as the rebuild-every-step path.
+int ljmd_forces_skincell(md_sim *s, bool energy)
+{
+    int r = vl_alloc_base(s);
+    if (r) return r;
+    if ((r = vl_decide_and_sort(s, LAYOUT_SKINCELL))) return r;
+    ljmd_tick(s, TAG_BUILD);
+    return ljmd_forces_cell2_on(s, s->vgrid, 0.5 * s->skin, energy, false);
+}
+
+// Decide, (re)build if the device-side flag says so, evaluate forces from the lists.
+int ljmd_forces_verlet(md_sim *s)
+{
+    int r = vl_alloc(s);
+    if (r) return r;
+    const int N = (int)s->N, nbl = (N + VL_T - 1) / VL_T;
+    const Grid &g = s->vgrid;
+    if ((r = vl_decide_and_sort(s, LAYOUT_VERLET))) return r;
     const double rl = s->rc + s->skin;
     if (s->vl_naive_build) {
         k_vl_build<<<nbl, VL_T, 0, s->stream>>>(s->lpos, s->cell_start, N, s->vl_npad, g, (float)(rl * rl), s->vl_cap, s->vl_list,
