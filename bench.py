@@ -370,8 +370,8 @@ def cpu_baseline_md(sysd, state, algo, budget_steps, threads):
 
 
 def bench_extras(b, torch, sysd, steps):
-    """Throughput of the (f3) extensions on the config-3 system: md_init_velocities and md_step with the
-    Andersen thermostat on (rand48 consumed in registers)."""
+    """Throughput of the SURVEY 8(f) extensions on the config-3 system: md_init_velocities and md_step with the
+    Andersen thermostat on (rand48 consumed in registers), skin cells, and the Yukawa pair potential."""
     N = sysd["N"]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     out = {}
@@ -397,6 +397,32 @@ def bench_extras(b, torch, sysd, steps):
         ms = e0.elapsed_time(e1) / steps
         out["md_step_andersen_cell"] = {"N": N, "ms_per_step": ms, "atom_steps_per_s": N / (ms * 1e-3),
                                         "note": "nu dt = 0.05; direct launches (no CUDA graph) with the thermostat on"}
+    # (f2) skin cells: the same system with cells of side >= rc + 0.3 re-sorted on the device's decision
+    with b.Sim(N, sysd["L"]) as s:
+        s.option("cell_skin", 0.3)
+        s.set_state(sysd["pos"], sysd["vel"])
+        s.step(sysd["steps"], 1)
+        nb0, ns0 = s.stat("vl_builds"), s.stat("vl_steps")
+        e0.record()
+        s.step(2 * steps, 1)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / (2 * steps)
+        out["md_step_skin_cells"] = {"N": N, "ms_per_step": ms, "atom_steps_per_s": N / (ms * 1e-3), "skin": 0.3,
+                                     "resorts_per_100_steps": 100.0 * (s.stat("vl_builds") - nb0) / max(1.0, s.stat("vl_steps") - ns0)}
+    # (f4) second pair potential: screened Coulomb (Yukawa), every in-range pair in FP64, on the three paths
+    for label, algo in (("cell", 1), ("verlet", 2)):
+        with b.Sim(N, sysd["L"]) as s:
+            s.potential(b.MD_POT_YUKAWA, 6.0, 1.2)
+            s.set_state(sysd["pos"], sysd["vel"])
+            s.step(100, algo)
+            e0.record()
+            s.step(steps, algo)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / steps
+            out["md_step_yukawa_" + label] = {"N": N, "ms_per_step": ms, "atom_steps_per_s": N / (ms * 1e-3),
+                                              "potential": "U = 6 exp(-1.2 r) / r, rc = 2.5, energy-shifted"}
     return out
 
 
@@ -529,7 +555,7 @@ def measure(args, b, torch, dist, rank, local_rank, world):
                                              "list_builds_per_100_steps": rv.get("vl_builds_per_100"),
                                              "roofline": vr}
             if oname == "c3_cell_256k":
-                others["f3_extensions_c3"] = bench_extras(b, torch, osys, osteps)
+                others["extensions_c3"] = bench_extras(b, torch, osys, osteps)
         others["c5_rand48"] = bench_rand48(b, torch, 5, peaks, True)
         line["others"] = others
     return line

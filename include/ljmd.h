@@ -48,6 +48,7 @@ typedef enum md_status {
  * enlarged for the next attempt). */
 enum { MD_ALLPAIRS = 0, MD_CELL = 1, MD_VERLET = 2 };
 enum { MD_TRUNCATED = 0, MD_ENERGY_SHIFTED = 1, MD_FORCE_SHIFTED = 2 }; /* shifted */
+enum { MD_POT_LJ = 0, MD_POT_YUKAWA = 1 };                                /* md_set_potential */
 enum { R48_U32_HI32 = 0, R48_U32_HI31 = 1, R48_F64 = 2, R48_U64_STATE = 3 }; /* kind */
 
 /* Create a simulation of N atoms in a cubic periodic box of side L with the Lennard-Jones
@@ -116,6 +117,17 @@ const char *md_strerror(int code);
 
 /* Stream (a cudaStream_t passed as void*) on which this handle's kernels run. */
 int md_set_stream(md_sim *s, void *cuda_stream);
+/* Another pair potential through the same machinery (an extension: PAPER.md:184, Outlook, "it is trivial to
+ * replace this potential by other pair-potentials, including the coulombic interaction").
+ *   MD_POT_LJ      Lennard-Jones with the eps, sigma of md_create (a, b ignored); the default.
+ *   MD_POT_YUKAWA  screened Coulomb between equal charges, U(r) = a exp(-b r) / r, f = -dU/dr
+ *                  (b = 0: the bare Coulomb pair a / r), truncated at the rc of md_create, with the same
+ *                  meaning of `shifted` (1: U - U(rc); 2: f - f(rc) and the matching U).  Every in-range
+ *                  pair is evaluated in FP64 on all three force paths (the FP32 fast branch of the cell and
+ *                  neighbour-list kernels exists for Lennard-Jones only, so those paths run slower).
+ * Marks the forces stale.  MD_EINVAL for an unknown kind, non-finite a or b, or b < 0. */
+int md_set_potential(md_sim *s, int kind, double a, double b);
+
 /* The same on an explicit CUDA stream (no process-wide state involved). */
 int rand48_fill_on(uint64_t *seeds, int64_t nstreams, int64_t ndraws, int kind, void *out, void *cuda_stream);
 

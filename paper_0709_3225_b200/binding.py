@@ -22,6 +22,7 @@ _alloc_keepalive = []
 MD_OK, MD_EINVAL, MD_EDOMAIN, MD_ESTATE, MD_ENOMEM, MD_ECUDA, MD_EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 MD_ALLPAIRS, MD_CELL, MD_VERLET = 0, 1, 2
 MD_TRUNCATED, MD_ENERGY_SHIFTED, MD_FORCE_SHIFTED = 0, 1, 2
+MD_POT_LJ, MD_POT_YUKAWA = 0, 1
 R48_U32_HI32, R48_U32_HI31, R48_F64, R48_U64_STATE = 0, 1, 2, 3
 R48_DTYPES = {0: np.uint32, 1: np.uint32, 2: np.float64, 3: np.uint64}
 
@@ -44,6 +45,7 @@ _SIGS = {
     "md_strerror": ([_i32], ctypes.c_char_p),
     "md_init_velocities": ([_vp, ctypes.c_double, ctypes.c_uint64], _i32),
     "md_set_stream": ([_vp, _vp], _i32),
+    "md_set_potential": ([_vp, _i32, _d, _d], _i32),
     "rand48_set_stream": ([_vp], _i32),
     "md_set_allocator": ([ALLOC_FN, FREE_FN], _i32),
     "md_set_option": ([_vp, ctypes.c_char_p, _d], _i32),
@@ -165,6 +167,10 @@ def md_init_velocities(h, T, seed48):
     _check(_lib.md_init_velocities(h, float(T), int(seed48)), "md_init_velocities")
 
 
+def md_set_potential(h, kind, a=0.0, b=0.0):
+    _check(_lib.md_set_potential(h, int(kind), float(a), float(b)), "md_set_potential")
+
+
 def md_set_stream(h, stream):
     _check(_lib.md_set_stream(h, stream), "md_set_stream")
 
@@ -253,6 +259,9 @@ class Sim:
 
     def energies(self):
         return md_get_energies(self.h)
+
+    def potential(self, kind, a=0.0, b=0.0):
+        md_set_potential(self.h, kind, a, b)
 
     def option(self, key, value):
         md_set_option(self.h, key, value)

@@ -30,6 +30,8 @@ struct PairParams {
     float rc2f_filter;     // FP32 accept threshold (rc^2 plus a rounding margin)
     float sig2f, eps24f, eps4f, ushiftf, rcf, f_rcf;
     int mode;
+    int kind;              // MD_POT_LJ or MD_POT_YUKAWA (md_set_potential)
+    double yA, ykappa;     // Yukawa: U = yA exp(-ykappa r) / r
 };
 
 // ---- cell grid on a power-of-two aligned lattice ----------
@@ -76,6 +78,8 @@ struct md_sim {
     int64_t N;
     double L, rc, eps, sigma, dt;
     int shifted;
+    int pot_kind;         // md_set_potential
+    double pot_a, pot_b;
     float Lf, dtf, hdtf;
     PairParams pp;
     Grid grid;            // grid.n == 0 when the box has fewer than 3 cells per dimension

@@ -74,6 +74,20 @@ __device__ __forceinline__ void f3_pair64(const PairParams &P, double dx, double
 {
     const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
     const bool in = r2 < P.rc2 && r2 > 0.0;              // strict
+    if (P.kind == 1) {                                   // Yukawa (pair.cuh): rare path, a branch is fine
+        if (in && r2 > 0.0) {
+            double fr_, u_;
+            yukawa_fu64(P, r2, fr_, u_);
+            fx = fma(-fr_, dx, fx);
+            fy = fma(-fr_, dy, fy);
+            fz = fma(-fr_, dz, fz);
+            if (ENERGY) {
+                pe += u_;
+                w = fma(fr_, r2, w);
+            }
+        }
+        return;
+    }
     const double inv = in ? rcp_f64(r2) : 0.0;
     const double s2 = P.sig2 * inv;
     const double s6 = s2 * s2 * s2;

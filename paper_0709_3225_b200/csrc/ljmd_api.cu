@@ -137,7 +137,16 @@ static void setup_pair(md_sim *s)
     P.ushift = (s->shifted >= 1) ? 4.0 * eps * (s6 * s6 - s6) : 0.0;
     P.f_rc = (s->shifted == 2) ? 24.0 * eps * (2.0 * s6 * s6 - s6) / rc : 0.0;
     P.mode = s->shifted;
-    P.precise_r2 = 1.3 * sg * sg;       // cell path: FP64 below this r^2
+    P.kind = s->pot_kind;
+    P.yA = s->pot_a;
+    P.ykappa = s->pot_b;
+    if (!s->precise_r2_user) P.precise_r2 = 1.3 * sg * sg;       // cell path: FP64 below this r^2
+    if (s->pot_kind == MD_POT_YUKAWA) {
+        const double e = s->pot_a * exp(-s->pot_b * rc) / rc;       // U_Y(rc), f_Y(rc) = U_Y (1/rc + kappa)
+        P.ushift = (s->shifted >= 1) ? e : 0.0;
+        P.f_rc = (s->shifted == 2) ? e * (1.0 / rc + s->pot_b) : 0.0;
+        P.precise_r2 = 1.0e300;         // every in-range pair in FP64: the FP32 fast branch is Lennard-Jones only
+    }
     // FP32 filter threshold: rc^2 plus the worst-case rounding error of an FP32 r^2 computed
     // from box-scale coordinates (|d| error <= 2 ulp(L)), so the filter never rejects a pair
     // that is inside rc in exact arithmetic.
@@ -323,6 +332,24 @@ extern "C" int md_destroy(md_sim *s)
     cudaStreamSynchronize(s->stream);
     free_all(s);
     delete s;
+    return MD_OK;
+}
+
+extern "C" int md_set_potential(md_sim *s, int kind, double a, double b)
+{
+    if (!s) return MD_EINVAL;
+    if (kind != MD_POT_LJ && kind != MD_POT_YUKAWA) return MD_EINVAL;
+    if (kind == MD_POT_YUKAWA && (!isfinite(a) || !isfinite(b) || b < 0.0)) return MD_EINVAL;
+    CK(cudaStreamSynchronize(s->stream));
+    const bool was_yukawa = s->pot_kind == MD_POT_YUKAWA;
+    s->pot_kind = kind;
+    s->pot_a = a;
+    s->pot_b = b;
+    if (kind == MD_POT_YUKAWA) s->precise_r2_user = true;          // the window stays as set below
+    else if (was_yukawa) s->precise_r2_user = false;
+    setup_pair(s);
+    s->forces_valid = false;
+    drop_graphs(s);
     return MD_OK;
 }
 

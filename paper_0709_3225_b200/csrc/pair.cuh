@@ -19,6 +19,25 @@ __device__ __forceinline__ double rcp_f64(double x)
     return y;
 }
 
+// Second pair potential ("trivial to replace this potential by other
+// pair-potentials, including the coulombic interaction"): screened Coulomb (Yukawa) between equal charges,
+//   U_Y = A exp(-kappa r) / r,   f_Y = -dU_Y/dr = U_Y (1/r + kappa),
+// the bare Coulomb pair for kappa = 0; same cutoff and shift modes (ushift = U_Y(rc), f_rc = f_Y(rc)).
+// Evaluated in FP64 on every path (md_set_potential makes the FP32 window of the cell and list kernels empty).
+// U and f/r of a pair inside rc:
+__device__ __forceinline__ void yukawa_fu64(const PairParams &P, double r2, double &fr, double &u)
+{
+    const double r = sqrt(r2), ir = 1.0 / r;
+    const double e = P.yA * exp(-P.ykappa * r) * ir;
+    double f = e * (ir + P.ykappa);
+    u = e - P.ushift;
+    if (P.mode == 2) {
+        u += (r - P.rc) * P.f_rc;
+        f -= P.f_rc;
+    }
+    fr = f * ir;
+}
+
 // FP64 pair term.  d = r_j - r_i (minimum image applied).  Returns true when r2 < rc^2
 // (strict) and then adds this pair's contribution:  F_i -= (f/r) d  (Eq. 1),
 // pe += U, w += r f.  Callers halve pe and w when they visit each pair twice.
@@ -27,6 +46,16 @@ __device__ __forceinline__ bool pair_f64(const PairParams &P, double dx, double 
 {
     double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
     if (!(r2 < P.rc2)) return false;
+    if (P.kind == 1) {
+        double fr, u;
+        yukawa_fu64(P, r2, fr, u);
+        fx = fma(-fr, dx, fx);
+        fy = fma(-fr, dy, fy);
+        fz = fma(-fr, dz, fz);
+        pe += u;
+        w = fma(fr, r2, w);
+        return true;
+    }
     double inv = rcp_f64(r2);
     double s2 = P.sig2 * inv;
     double s6 = s2 * s2 * s2;
