@@ -458,12 +458,13 @@ def measure(args, b, torch, dist, rank, local_rank, world):
         algo = b.MD_VERLET
     buf = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")
     steps, warmup = args.steps, max(3, args.warmup)
+    opts = {kv.split("=", 1)[0]: float(kv.split("=", 1)[1]) for kv in args.opt}
 
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
     with ClockSampler(local_rank) as clk:
-        r = time_md(b, torch, sysd, algo, steps, warmup, True, buf)
+        r = time_md(b, torch, sysd, algo, steps, warmup, True, buf, options=opts)
     ms = r["flushed_ms"]
     e2e = time_md_e2e(b, torch, sysd, r["melted"], algo, min(steps, 50), 1)
     e2e10 = time_md_e2e(b, torch, sysd, r["melted"], algo, max(2, min(steps, 50) // 5), 10)
@@ -497,7 +498,7 @@ def measure(args, b, torch, dist, rank, local_rank, world):
                    "algo": ("allpairs", "cell", "verlet")[algo], "shifted": wl.SHIFTED,
                    "state": "fcc lattice + md_init_velocities, advanced %d steps (the config's length) before timing" % cfg["steps"],
                    "l2": "flushed between steps (256 MB read-modify-write); steady_state is the unflushed md_step(K) loop",
-                   "stream": "PyTorch side stream, PyTorch caching allocator",
+                   "stream": "PyTorch side stream, PyTorch caching allocator", "options": opts,
                    "parallelism": "replicas x%d" % world if world > 1 else "single GPU"},
         "steady_state": {"ms_per_step": r["steady_ms"], "value": world * N / (r["steady_ms"] * 1e-3)},
         "phases_ms": r["phases_ms"],
@@ -606,6 +607,8 @@ def main():
     ap.add_argument("--algo", default=None, choices=["verlet"],
                     help="run the workload's system through the neighbour-list path instead of its named path")
     ap.add_argument("--no-others", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="md_set_option for the headline workload, e.g. --opt cell_kernel=3 (repeatable)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
