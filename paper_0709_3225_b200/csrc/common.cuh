@@ -137,6 +137,7 @@ struct md_sim {
     uint32_t and_thr;
     double and_T, and_nu;
     uint64_t and_seed, and_t;     // stream start state, steps since it was (re)configured
+    uint64_t *and_t_dev;          // the same count in device memory (read by the thermostat kernel, graph-replayable)
     bool precise_r2_user;         // "precise_r2" was set through md_set_option
     int cell_group;               // cells per row group of the cell-force kernel; 0 = automatic
     int cell_kernel;              // 2 (default): force_cell2.cu; 3: force_cell3.cu (dense); 1: force_cell.cu

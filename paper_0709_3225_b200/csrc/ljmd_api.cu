@@ -215,7 +215,7 @@ static void free_all(md_sim *s)
     free(s->ev_pool);
     free(s->ev_tag);
     void *ptrs[] = {s->pos, s->vel, s->frc, s->pos2, s->vel2, s->lpos, s->cell_of, s->rank, s->cell_count,
-                    s->cell_start, s->max_occ, s->scan_ctl, s->scan_state, s->vl_list, s->vl_count, s->vl_lbuild, s->vl_ctl, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list,
+                    s->cell_start, s->max_occ, s->scan_ctl, s->scan_state, s->vl_list, s->vl_count, s->vl_lbuild, s->vl_ctl, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list, s->and_t_dev,
                     s->tile_start};
     for (void *p : ptrs) ljmd_dev_free(p, st);
 }
@@ -293,12 +293,13 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->fpart = (double *)ljmd_dev_alloc((size_t)nsplit * 3 * N * sizeof(double), st);
     s->part = (double *)ljmd_dev_alloc((size_t)3 * s->part_cap * sizeof(double), st);
     s->energies = (double *)ljmd_dev_alloc(3 * sizeof(double), st);
+    s->and_t_dev = (uint64_t *)ljmd_dev_alloc(sizeof(uint64_t), st);
     s->xfer = (float *)ljmd_dev_alloc((size_t)N * 3 * sizeof(float), st);
     int ntiles = s->ap_sort_bins > 0 ? s->ap_sort_bins : 1;
     s->tile_count = (int *)ljmd_dev_alloc((size_t)ntiles * sizeof(int), st);
     s->tile_start = (int *)ljmd_dev_alloc(((size_t)ntiles + 1) * sizeof(int), st);
     if (!s->tile_count || !s->tile_start || !s->pos || !s->vel || !s->frc || !s->pos2 || !s->vel2 || !s->lpos || !s->cell_of || !s->rank ||
-        !s->cell_count || !s->cell_start || !s->max_occ || !s->scan_ctl || !s->scan_state || !s->fpart || !s->part || !s->energies || !s->xfer) {
+        !s->cell_count || !s->cell_start || !s->max_occ || !s->scan_ctl || !s->scan_state || !s->fpart || !s->part || !s->energies || !s->xfer || !s->and_t_dev) {
         free_all(s);
         delete s;
         return MD_ENOMEM;
@@ -315,6 +316,7 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     if (e == cudaSuccess) e = cudaMemsetAsync(s->scan_state, 0, (size_t)s->scan_cap * sizeof(unsigned long long), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->tile_count, 0, (size_t)ntiles * sizeof(int), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->frc, 0, f4, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->and_t_dev, 0, sizeof(uint64_t), st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) {
         ljmd_note_cuda_error(e, "md_create init", __FILE__, __LINE__);
@@ -521,6 +523,18 @@ static int one_step(md_sim *s, int algo, int kicks, bool last, bool energy, bool
     return MD_OK;
 }
 
+// One interior step of md_step (neither the first nor the last of the call).  With the Andersen thermostat the
+// collisions follow every second half-kick, so nothing is folded into the next step and nothing is fused.
+static int interior_step(md_sim *s, int algo)
+{
+    if (!s->and_thr) return one_step(s, algo, 2, false, false);
+    int r = one_step(s, algo, 1, false, false, false);
+    if (r) return r;
+    if ((r = ljmd_kick_andersen(s))) return r;
+    ljmd_tick(s, TAG_INTEGRATE);
+    return MD_OK;
+}
+
 // Steps after which the host-side state repeats: the cell build swaps the pos/vel buffer roles
 // every step; the all-pairs path re-sorts (and swaps) every sort_every steps.
 static int graph_unit(const md_sim *s, int algo)
@@ -572,7 +586,7 @@ static int replay_interior(md_sim *s, int algo, int unit, int64_t nunits, int64_
         int r = MD_OK;
         if (cudaStreamBeginCapture(run, cudaStreamCaptureModeThreadLocal) != cudaSuccess) r = MD_ECUDA;
         if (r == MD_OK) {
-            for (int q = 0; q < unit && r == MD_OK; q++) r = one_step(s, algo, 2, false, false);
+            for (int q = 0; q < unit && r == MD_OK; q++) r = interior_step(s, algo);
             cudaError_t ce = cudaStreamEndCapture(run, &graph);
             if (ce != cudaSuccess || !graph) r = MD_ECUDA;
         }
@@ -583,6 +597,7 @@ static int replay_interior(md_sim *s, int algo, int unit, int64_t nunits, int64_
         e.launches = s->launches - l0;
         s->stream = user;
         s->launches = l0;
+        s->and_t = saved.and_t;                          // nothing ran during the capture
         if (r != MD_OK || !same) {
             // nothing was executed during the capture: put the host state back and go on without graphs
             cudaGetLastError();
@@ -604,6 +619,7 @@ static int replay_interior(md_sim *s, int algo, int unit, int64_t nunits, int64_
     for (int64_t u = 0; u < nunits; u++) {
         CK(cudaGraphLaunch(g->exec, run));
         s->launches += g->launches;
+        if (s->and_thr) s->and_t += (uint64_t)unit;
     }
     s->graph_replays += nunits;
     if (algo == MD_CELL) s->binned = false;
@@ -665,15 +681,7 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
     // Interior steps (all but the first and the last) are identical launch sequences and are
     // replayed from a CUDA graph, one unit of steps per replay.
     int64_t k = 0;
-    if (s->and_thr) {
-        // Andersen thermostat: the collisions follow every second half-kick, so nothing is folded into
-        // the next step and the step index is a kernel argument (direct launches, no graph)
-        for (; k < nsteps; k++) {
-            if ((r = one_step(s, algo, 1, false, k == nsteps - 1, false))) return r;
-            if ((r = ljmd_kick_andersen(s))) return r;
-            ljmd_tick(s, TAG_INTEGRATE);
-        }
-    }
+    const bool thermo = s->and_thr != 0;         // Andersen thermostat: see interior_step; the step index lives on the device
     while (k < nsteps) {
         if (k > 0 && k < nsteps - 1 && s->use_graph && !s->time_kernels) {
             const int unit = graph_unit(s, algo);
@@ -684,7 +692,11 @@ extern "C" int md_step(md_sim *s, int64_t nsteps, int algo)
                 if (done) continue;
             }
         }
-        if ((r = one_step(s, algo, (k > 0) ? 2 : 1, k == nsteps - 1, k == nsteps - 1))) return r;
+        if (thermo) {
+            if ((r = one_step(s, algo, 1, false, k == nsteps - 1, false))) return r;
+            if ((r = ljmd_kick_andersen(s))) return r;
+            ljmd_tick(s, TAG_INTEGRATE);
+        } else if ((r = one_step(s, algo, (k > 0) ? 2 : 1, k == nsteps - 1, k == nsteps - 1))) return r;
         k++;
     }
     if ((r = ljmd_reduce_energies(s))) return r;
@@ -746,6 +758,7 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
         if (thr > 4294967295.0) thr = 4294967295.0;
         s->and_thr = (s->and_T > 0) ? (uint32_t)thr : 0u;
         s->and_t = 0;                                                 // the stream starts over
+        CK(cudaMemsetAsync(s->and_t_dev, 0, sizeof(uint64_t), s->stream));
     } else if (!strcmp(key, "vl_naive_build")) {
         s->vl_naive_build = value != 0.0;
     } else if (!strcmp(key, "skin")) {

@@ -351,9 +351,11 @@ int ljmd_mb_velocities(md_sim *s, double T, uint64_t seed48, double *vraw, doubl
 // collision iff the 32 high bits of the first are < thr; the new velocity is computed in FP64.
 __global__ void __launch_bounds__(MB_T)
 k_kick_andersen(float4 *__restrict__ vel, const float4 *__restrict__ frc, const float4 *__restrict__ pos, int64_t N,
-                float hdt, double sqrtT, uint32_t thr, uint64_t seed, uint64_t t, double *__restrict__ part_ke)
+                float hdt, double sqrtT, uint32_t thr, uint64_t seed, const uint64_t *__restrict__ tptr,
+                double *__restrict__ part_ke)
 {
     __shared__ double red[32];
+    const uint64_t t = *tptr;                            // step index, in device memory: the launch can sit in a graph
     const int64_t slot = (int64_t)blockIdx.x * MB_T + threadIdx.x;
     double ke = 0.0;
     if (slot < N) {
@@ -384,6 +386,8 @@ k_kick_andersen(float4 *__restrict__ vel, const float4 *__restrict__ frc, const 
     if (threadIdx.x == 0) part_ke[blockIdx.x] = ke;
 }
 
+__global__ void __launch_bounds__(1) k_andersen_tick(uint64_t *t) { *t += 1ull; }
+
 int ljmd_kick_andersen(md_sim *s)
 {
     cudaStream_t st = s->stream;
@@ -393,7 +397,9 @@ int ljmd_kick_andersen(md_sim *s)
     }
     const int nb = (int)((s->N + MB_T - 1) / MB_T);
     k_kick_andersen<<<nb, MB_T, 0, st>>>(s->vel, s->frc, s->pos, s->N, s->hdtf, sqrt(s->and_T), s->and_thr, s->and_seed,
-                                         s->and_t, s->part);
+                                         s->and_t_dev, s->part);
+    CKL(s);
+    k_andersen_tick<<<1, 1, 0, st>>>(s->and_t_dev);
     CKL(s);
     s->n_ke = nb;
     s->and_t++;

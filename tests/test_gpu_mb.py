@@ -57,21 +57,26 @@ def test_config1_pin_and_errors(b):
             assert e.value.code == b.MD_EINVAL
 
 
+@pytest.mark.parametrize("graph", [1, 0])
 @pytest.mark.parametrize("algo", [0, 1, 2])
-def test_andersen_thermostat_matches_the_oracle(b, algo, oracle_uniforms):
-    """30 steps with collisions (nu dt = 0.05) on config 1 against the oracle's step + andersen_collide."""
+def test_andersen_thermostat_matches_the_oracle(b, algo, graph, oracle_uniforms):
+    """30 steps with collisions (nu dt = 0.05) on config 1 against the oracle's step + andersen_collide; the
+    interior steps of a call are replayed from a CUDA graph (the step index lives in device memory) or launched
+    directly."""
     c1 = wl.md_system("c1_allpairs_500", velocities_from(oracle_uniforms))
     N, L, T, nu, seed = c1["N"], c1["L"], 1.5, 10.0, 0x0123456789AB
     with b.Sim(N, L) as s:
         s.option("andersen_T", T)
         s.option("andersen_seed", seed)
         s.option("andersen_nu", nu)
+        s.option("graph", graph)
         thr = int(s.stat("andersen_threshold"))
         assert thr == int(np.floor(nu * 0.005 * 2.0 ** 32))
         s.set_state(c1["pos"], c1["vel"])
         s.step(12, algo)
         s.step(18, algo)                                   # the step index carries over between calls
         assert s.stat("andersen_steps") == 30
+        assert (s.stat("graph_replays") > 0) == bool(graph)
         p, v = s.get_state()
         ke, pe, w = s.energies()
     po, vo = c1["pos"].astype(np.float64), c1["vel"].astype(np.float64)
