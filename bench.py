@@ -410,6 +410,17 @@ def bench_extras(b, torch, sysd, steps):
         ms = e0.elapsed_time(e1) / (2 * steps)
         out["md_step_skin_cells"] = {"N": N, "ms_per_step": ms, "atom_steps_per_s": N / (ms * 1e-3), "skin": 0.3,
                                      "resorts_per_100_steps": 100.0 * (s.stat("vl_builds") - nb0) / max(1.0, s.stat("vl_steps") - ns0)}
+    # neighbour lists with Newton's third law (option "vl_half"): every pair once, reactions through reductions
+    with b.Sim(N, sysd["L"]) as s:
+        s.option("vl_half", 1)
+        s.set_state(sysd["pos"], sysd["vel"])
+        s.step(sysd["steps"], 2)
+        e0.record()
+        s.step(2 * steps, 2)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / (2 * steps)
+        out["md_step_verlet_half_lists"] = {"N": N, "ms_per_step": ms, "atom_steps_per_s": N / (ms * 1e-3)}
     # (f4) second pair potential: screened Coulomb (Yukawa), every in-range pair in FP64, on the three paths
     for label, algo in (("cell", 1), ("verlet", 2)):
         with b.Sim(N, sysd["L"]) as s:

@@ -158,6 +158,11 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
  *                    high bits).  Active once nu > 0 and T > 0; nu = 0 switches it off.  Steps are then
  *                    launched directly (no graph, no folded half-kick).
  *   "skin"           MD_VERLET: list radius minus rc (default 0.3 sigma); only before the first use
+ *   "cell_skin"      MD_CELL on skin cells: cells of side >= rc + value, re-sorted on the device's own
+ *                    decision when an atom has strayed value / 2; 0 (default) = the cell
+ *                    list is rebuilt every step.  Shares the skin with MD_VERLET (set before either runs)
+ *   "vl_half"        MD_VERLET with half lists: every pair once, the reaction force through vector
+ *                    reductions (default 0; measured in DESIGN.md section 7b)
  *   "cell_group"     cells of one z-column handled by one warp of the cell-force kernel (1..5);
  *                    0 (default) = chosen from the mean occupancy
  *   "time_kernels"   1 = record CUDA events around every phase of md_step (disables the graph);

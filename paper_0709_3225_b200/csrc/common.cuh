@@ -90,6 +90,7 @@ struct md_sim {
     float4 *vl_lbuild;    // [N] local coordinates at the last build
     VlCtl *vl_ctl;
     int vl_cap, vl_npad;
+    bool vl_half;         // option "vl_half": half lists + vector reductions for the reactions (measurement)
     bool vl_naive_build;  // option "vl_naive_build": thread-per-atom list kernel instead of the warp filter
     int grid_paper_n;     // int[L/rc]
     cudaStream_t stream;

@@ -759,6 +759,9 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
         s->and_thr = (s->and_T > 0) ? (uint32_t)thr : 0u;
         s->and_t = 0;                                                 // the stream starts over
         CK(cudaMemsetAsync(s->and_t_dev, 0, sizeof(uint64_t), s->stream));
+    } else if (!strcmp(key, "vl_half")) {
+        s->vl_half = value != 0.0;
+        s->layout = LAYOUT_NONE;                        // rebuild the lists in the other form
     } else if (!strcmp(key, "vl_naive_build")) {
         s->vl_naive_build = value != 0.0;
     } else if (!strcmp(key, "skin")) {

@@ -181,7 +181,7 @@ k_vl_copyback(float4 *__restrict__ pos, float4 *__restrict__ vel, float4 *__rest
 // local coordinates.  list[k * npad + i] = slot of j | offset-table index << 23.
 __global__ void __launch_bounds__(VL_T)
 k_vl_build(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, int N, int npad, Grid g, float rl2,
-           int cap, unsigned *__restrict__ list, int *__restrict__ count, VlCtl *__restrict__ ctl)
+           int cap, unsigned *__restrict__ list, int *__restrict__ count, VlCtl *__restrict__ ctl, int half)
 {
     if (!ctl->rebuild) return;
     const int i = blockIdx.x * VL_T + threadIdx.x;
@@ -212,7 +212,7 @@ k_vl_build(const float4 *__restrict__ lpos, const int *__restrict__ cell_start, 
                     const float4 lj = lpos[j];
                     const float dx = (lj.x - li.x) + ox, dy = (lj.y - li.y) + oy, dz = (lj.z - li.z) + oz;
                     const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                    if (r2 < rl2 && j != i) {
+                    if (r2 < rl2 && j != i && (!half || j > i)) {      // half lists: each pair once, in the lower slot's list
                         if (cnt < cap) list[(size_t)cnt * npad + i] = (unsigned)j | tag;
                         cnt++;
                     }
@@ -244,7 +244,16 @@ __device__ __forceinline__ void vl_precise(const float4 *__restrict__ lpos, cons
     pair_f64(P, ex, ey, ez, fx, fy, fz, pe, w);
 }
 
-template <bool MODE2>
+// reaction force of one pair on atom j: one vector reduction into the L2 (no return value)
+__device__ __forceinline__ void vl_react(float4 *frc, int j, float x, float y, float z)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" :: "l"(frc + j), "f"(x), "f"(y), "f"(z), "f"(0.f) : "memory");
+}
+
+// HALF (option "vl_half", a measurement of Newton's third law on this path): the lists hold
+// every pair once; the force on i is summed in registers and added to frc[i] at the end, the reaction goes to
+// frc[j] pair by pair through red.global.add.v4.f32; frc is zeroed before the launch.
+template <bool MODE2, bool HALF>
 __global__ void __launch_bounds__(VL_T, VL_MINB)
 k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams P, VlConst K,
            const unsigned *__restrict__ list, const int *__restrict__ count, float4 *__restrict__ frc,
@@ -301,6 +310,7 @@ k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams 
                 fx = fmaf(-fr, dx, fx);
                 fy = fmaf(-fr, dy, fy);
                 fz = fmaf(-fr, dz, fz);
+                if (HALF && fast) vl_react(frc, (int)(e[u] & VL_JMASK), fr * dx, fr * dy, fr * dz);
                 sA = fmaf(s6, s6, sA);
                 sB += s6;
                 nin += fast ? 1 : 0;
@@ -309,7 +319,13 @@ k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams 
         // FP64 part: the queued pairs; a thread whose queue overflowed rescans its list instead
         double dfx = 0.0, dfy = 0.0, dfz = 0.0, dpe = 0.0, dw = 0.0;
         if (nq <= VL_Q) {
-            for (int q = 0; q < nq; q++) vl_precise(lpos, offt, P, li, queue[q][threadIdx.x], dfx, dfy, dfz, dpe, dw);
+            for (int q = 0; q < nq; q++) {
+                const unsigned e = queue[q][threadIdx.x];
+                double px = 0.0, py = 0.0, pz = 0.0;
+                vl_precise(lpos, offt, P, li, e, px, py, pz, dpe, dw);
+                dfx += px; dfy += py; dfz += pz;
+                if (HALF) vl_react(frc, (int)(e & VL_JMASK), (float)-px, (float)-py, (float)-pz);
+            }
         } else {
             row = list + i;
             for (int k = 0; k < cnt; k++) {
@@ -318,10 +334,16 @@ k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams 
                 const float4 o = offt[e >> 23];
                 const float dx = (lj.x - li.x) + o.x, dy = (lj.y - li.y) + o.y, dz = (lj.z - li.z) + o.z;
                 const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                if (!(r2 >= K.p2 && r2 < K.rc2_lo) && r2 < K.rc2_hi) vl_precise(lpos, offt, P, li, e, dfx, dfy, dfz, dpe, dw);
+                if (!(r2 >= K.p2 && r2 < K.rc2_lo) && r2 < K.rc2_hi) {
+                    double px = 0.0, py = 0.0, pz = 0.0;
+                    vl_precise(lpos, offt, P, li, e, px, py, pz, dpe, dw);
+                    dfx += px; dfy += py; dfz += pz;
+                    if (HALF) vl_react(frc, (int)(e & VL_JMASK), (float)-px, (float)-py, (float)-pz);
+                }
             }
         }
-        frc[i] = make_float4((float)(dfx + (double)fx), (float)(dfy + (double)fy), (float)(dfz + (double)fz), 0.f);
+        if (HALF) vl_react(frc, i, (float)(dfx + (double)fx), (float)(dfy + (double)fy), (float)(dfz + (double)fz));
+        else frc[i] = make_float4((float)(dfx + (double)fx), (float)(dfy + (double)fy), (float)(dfz + (double)fz), 0.f);
         pe = dpe + P.eps4 * ((double)sA - (double)sB) - (double)nin * P.ushift;
         w = dw + P.eps24 * (2.0 * (double)sA - (double)sB);
         if (MODE2) {
@@ -332,8 +354,8 @@ k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams 
     pe = block_sum(pe, red);
     w = block_sum(w, red);
     if (threadIdx.x == 0) {
-        part_pe[blockIdx.x] = 0.5 * pe;              // every pair is in both atoms' lists
-        part_w[blockIdx.x] = 0.5 * w;
+        part_pe[blockIdx.x] = (HALF ? 1.0 : 0.5) * pe;              // full lists: every pair is in both atoms' lists
+        part_w[blockIdx.x] = (HALF ? 1.0 : 0.5) * w;
     }
 }
 
@@ -469,9 +491,9 @@ int ljmd_forces_verlet(md_sim *s)
     const Grid &g = s->vgrid;
     if ((r = vl_decide_and_sort(s, LAYOUT_VERLET))) return r;
     const double rl = s->rc + s->skin;
-    if (s->vl_naive_build) {
+    if (s->vl_naive_build || s->vl_half) {
         k_vl_build<<<nbl, VL_T, 0, s->stream>>>(s->lpos, s->cell_start, N, s->vl_npad, g, (float)(rl * rl), s->vl_cap, s->vl_list,
-                                                s->vl_count, s->vl_ctl);
+                                                s->vl_count, s->vl_ctl, s->vl_half ? 1 : 0);
         CKL(s);
     } else if ((r = ljmd_vl_build_lists(s, &s->vl_ctl->rebuild))) return r;
     ljmd_tick(s, TAG_BUILD);
@@ -491,15 +513,19 @@ int ljmd_forces_verlet(md_sim *s)
         // (30 % still holds eight blocks' tables and queues); measured 3 % faster than the default split
         static bool carved = false;
         if (!carved) {
-            cudaFuncSetAttribute(k_vl_force<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
-            cudaFuncSetAttribute(k_vl_force<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
+            cudaFuncSetAttribute(k_vl_force<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
+            cudaFuncSetAttribute(k_vl_force<true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
+            cudaFuncSetAttribute(k_vl_force<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
+            cudaFuncSetAttribute(k_vl_force<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
             carved = true;
         }
     }
-    if (P.mode == 2)
-        k_vl_force<true><<<nbl, VL_T, 0, s->stream>>>(s->lpos, N, s->vl_npad, g, P, K, s->vl_list, s->vl_count, s->frc, ppe, pw);
-    else
-        k_vl_force<false><<<nbl, VL_T, 0, s->stream>>>(s->lpos, N, s->vl_npad, g, P, K, s->vl_list, s->vl_count, s->frc, ppe, pw);
+    if (s->vl_half) CK(cudaMemsetAsync(s->frc, 0, (size_t)N * sizeof(float4), s->stream));
+#define VL_LAUNCH(M2, H) \
+    k_vl_force<M2, H><<<nbl, VL_T, 0, s->stream>>>(s->lpos, N, s->vl_npad, g, P, K, s->vl_list, s->vl_count, s->frc, ppe, pw)
+    if (P.mode == 2) { if (s->vl_half) VL_LAUNCH(true, true); else VL_LAUNCH(true, false); }
+    else { if (s->vl_half) VL_LAUNCH(false, true); else VL_LAUNCH(false, false); }
+#undef VL_LAUNCH
     CKL(s);
     ljmd_tick(s, TAG_FORCE);
     s->n_pe = nbl;

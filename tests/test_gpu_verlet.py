@@ -192,3 +192,45 @@ def test_eps_sigma_not_one(b):
     tol = np.maximum(1e-4 * np.abs(Fo), 1e-5 * eps / sigma)
     assert np.all(np.abs(F - Fo) <= tol)
     assert pe == pytest.approx(peo, rel=1e-6) and w == pytest.approx(wo, rel=1e-6)
+
+
+@pytest.mark.parametrize("shifted", [0, 1, 2])
+@pytest.mark.parametrize("n,rho,amp", [(6, 0.8, 0.10), (7, 0.9, 0.08), (8, 0.3, 0.12), (10, 0.8, 0.1)])
+def test_half_lists_with_reaction_forces(b, n, rho, amp, shifted):
+    """Option "vl_half" (Newton's third law on this path: every pair once, the reaction through vector
+    reductions): same forces and energies as the oracle, from fresh lists and after steps on reused ones."""
+    pos, L = wl.perturbed_fcc(n, rho, amp, seed=900 + n)
+    Fo, peo, wo = oracle.forces(pos.astype(np.float64), L, mode=shifted, algo=0)
+    with b.Sim(pos.shape[0], L, shifted=shifted) as s:
+        s.option("vl_half", 1)
+        s.set_state(pos, np.zeros_like(pos))
+        s.compute_forces(b.MD_VERLET)
+        assert force_check(s.forces(), Fo)[0] == 0
+        _, pe, w = s.energies()
+        assert pe == pytest.approx(peo, rel=1e-6) and w == pytest.approx(wo, rel=1e-6)
+        s.step(15, b.MD_VERLET)
+        p, v = s.get_state()
+        assert np.all(np.isfinite(p))
+        Fo2, peo2, _ = oracle.forces(p.astype(np.float64), L, mode=shifted, algo=0)
+        assert force_check(s.forces(), Fo2)[0] == 0
+        assert s.energies()[1] == pytest.approx(peo2, rel=1e-6)
+
+
+def test_half_lists_full_size_c3(b):
+    import os
+    oracle.set_threads(os.cpu_count() or 1)
+
+    def src(seed48, n):
+        out, _ = b.rand48([seed48], n, b.R48_F64)
+        return out[0]
+    sysd = wl.md_system("c3_cell_256k", velocities_from(src))
+    with b.Sim(sysd["N"], sysd["L"]) as s:
+        s.option("vl_half", 1)
+        s.set_state(sysd["pos"], sysd["vel"])
+        s.step(1000, b.MD_VERLET)
+        ke, pe, w = s.energies()
+        F = s.forces()
+        p, v = s.get_state()
+    Fo, peo, wo = oracle.forces(p.astype(np.float64), sysd["L"], algo=1)
+    check_forces(F, Fo, p, sysd["L"], oracle)
+    assert pe == pytest.approx(peo, rel=1e-6) and w == pytest.approx(wo, rel=1e-6)
