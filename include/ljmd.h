@@ -78,10 +78,12 @@ int md_get_state(md_sim *s, float *pos, float *vel);
 int md_compute_forces(md_sim *s, int algo);
 
 /* Advance nsteps velocity-Verlet steps (order per R4): half-kick, drift with
- * periodic wrap, force evaluation with algo, half-kick.  If the forces are stale (or were
- * last evaluated by the other algo's data layout) they are evaluated first; that evaluation
- * is not a step.  MD_CELL rebuilds the cell list from current positions before every force
- * evaluation (R20).  nsteps = 0 is allowed.  Atoms moving more than L per step and
+ * periodic wrap, force evaluation with algo, half-kick.  If the forces are stale they are
+ * evaluated first with algo; that evaluation is not a step.  Forces last evaluated by another
+ * algo are reused as they are (all paths compute the same forces) except by the paths whose
+ * integrator needs their own data layout: MD_VERLET, and MD_CELL with "cell_skin", evaluate
+ * first when another path ran last.  MD_CELL rebuilds the cell list from current positions
+ * before every force evaluation (R20; "cell_skin" = 0).  nsteps = 0 is allowed.  Atoms moving more than L per step and
  * coincident atoms are undefined behaviour. */
 int md_step(md_sim *s, int64_t nsteps, int algo);
 
