@@ -178,6 +178,8 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
  *   "cell_kernel"    cell-force kernel: 2 (default) ballot filter + per-lane walk (force_cell2.cu),
  *                    1 its first version (force_cell.cu), 3 dense evaluation of every staged
  *                    candidate (force_cell3.cu); same forces within the tolerances of DESIGN.md 12
+ *   "cell_order"     1 = cells numbered along a Morton curve instead of linearly (dense kernel only: selects
+ *                    "cell_kernel" = 3; default 0: measured slower)
  *   "fuse_integrator" 1 = interior steps of md_step(MD_CELL) integrate in the force kernel's epilogue
  *                    (kernels 2 and 3; default 0: measured slower)
  *   "sort_every"     all-pairs path: re-sort atoms along the Hilbert curve every k steps (default 10)

@@ -255,7 +255,7 @@ k_bin3(const float4 *__restrict__ pos, float4 *__restrict__ vel, int N, Grid g, 
     int i = blockIdx.x * CB_T + threadIdx.x;
     if (i >= N) return;
     const float4 p = pos[i];
-    const int c = (cell_coord(p.x, g) * g.n + cell_coord(p.y, g)) * g.n + cell_coord(p.z, g);
+    const int c = cell_id(cell_coord(p.x, g), cell_coord(p.y, g), cell_coord(p.z, g), g);
     reinterpret_cast<int *>(vel)[4 * i + 3] = atomicAdd(&cell_count[c], 1);
 }
 
@@ -277,7 +277,7 @@ k_kick_drift_bin3(float4 *__restrict__ pos, float4 *__restrict__ vel, const floa
     p.x = wrap_drift(fmaf(dt, v.x, p.x), g.L);
     p.y = wrap_drift(fmaf(dt, v.y, p.y), g.L);
     p.z = wrap_drift(fmaf(dt, v.z, p.z), g.L);
-    const int c = (cell_coord(p.x, g) * g.n + cell_coord(p.y, g)) * g.n + cell_coord(p.z, g);
+    const int c = cell_id(cell_coord(p.x, g), cell_coord(p.y, g), cell_coord(p.z, g), g);
     v.w = __int_as_float(atomicAdd(&cell_count[c], 1));
     pos[i] = p;
     vel[i] = v;
@@ -292,12 +292,12 @@ k_scatter3(const float4 *__restrict__ pos, const float4 *__restrict__ vel, int N
     if (i >= N) return;
     const float4 p = pos[i];
     float4 v = vel[i];
-    const int c = (cell_coord(p.x, g) * g.n + cell_coord(p.y, g)) * g.n + cell_coord(p.z, g);
+    const int c = cell_id(cell_coord(p.x, g), cell_coord(p.y, g), cell_coord(p.z, g), g);
     const int dst = cell_start[c] + __float_as_int(v.w);
     v.w = 0.f;
     pos2[dst] = p;
     vel2[dst] = v;
-    if (lpos) {                                        // cell-local copy for the filter kernels (force_cell2.cu)
+    if (lpos) {                                        // cell-local copy for the filter kernels (force_cell2.cu); linear ids
         const int cz = c % g.n, cy = (c / g.n) % g.n, cx = c / (g.n * g.n);
         lpos[dst] = make_float4(p.x - (float)cx * g.side, p.y - (float)cy * g.side, p.z - (float)cz * g.side,
                                 __int_as_float(c));    // exact
@@ -331,7 +331,7 @@ int ljmd_cell_build3(md_sim *s)
     }
     s->binned3 = false;
     s->fused_pending = false;
-    int r = ljmd_scan_counts(s, s->cell_count, s->cell_start, s->grid.ncells);
+    int r = ljmd_scan_counts(s, s->cell_count, s->cell_start, s->grid.nid);
     if (r) return r;
     if (pending) {
         k_scatter3<<<nb, CB_T, 0, s->stream>>>(s->pos2, s->vel, N, s->grid, s->cell_start, s->pos, s->vel2, lp);

@@ -42,6 +42,8 @@ struct Grid {
     float last;       // width of cell n-1 = L - (n-1)*side  (>= side)
     float inv_side;
     float L;
+    int morton;       // option "cell_order" = 1 (dense kernel only): cells numbered along a Morton curve
+    int nid;          // number of cell ids: n^3, or P^3 with P = the power of two >= n for the Morton numbering
 };
 
 // One cached graph: valid for this force path and exactly this host-side state at the unit's start
@@ -212,6 +214,34 @@ __device__ __forceinline__ int cell_coord(float x, const Grid &g)
     if (x < o) c--;
     else if (c < g.n - 1 && x >= o + g.side) c++;
     return c;
+}
+
+// Cell number of cell (cx, cy, cz): linear (a z-column is one contiguous run of slots), or along a Morton curve
+// (north_star (b): "optional Morton or linear cell ordering"; ids of the padded cube P^3, unused ids stay empty).
+__host__ __device__ __forceinline__ unsigned morton_spread(unsigned v)
+{
+    v &= 0x3ffu;
+    v = (v | (v << 16)) & 0x030000ffu;
+    v = (v | (v << 8)) & 0x0300f00fu;
+    v = (v | (v << 4)) & 0x030c30c3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+
+__host__ __device__ __forceinline__ unsigned morton_compact(unsigned v)
+{
+    v &= 0x09249249u;
+    v = (v | (v >> 2)) & 0x030c30c3u;
+    v = (v | (v >> 4)) & 0x0300f00fu;
+    v = (v | (v >> 8)) & 0x030000ffu;
+    v = (v | (v >> 16)) & 0x3ffu;
+    return v;
+}
+
+__device__ __forceinline__ int cell_id(int cx, int cy, int cz, const Grid &g)
+{
+    if (g.morton) return (int)((morton_spread((unsigned)cx) << 2) | (morton_spread((unsigned)cy) << 1) | morton_spread((unsigned)cz));
+    return (cx * g.n + cy) * g.n + cz;
 }
 
 __device__ __forceinline__ double warp_sum(double v)

@@ -165,8 +165,14 @@ k_fc3(const float4 *__restrict__ pos, const int *__restrict__ cell_start, const 
     __shared__ __align__(16) F3Smem S;
     const int lane = threadIdx.x;
     const int n = g.n;
-    const int cz = blockIdx.x, cy = blockIdx.y, cx = blockIdx.z;
-    const int home = (cx * n + cy) * n + cz;
+    int cz = blockIdx.x, cy = blockIdx.y, cx = blockIdx.z;
+    if (g.morton) {                                      // 1-D grid over the padded cube, blocks in Morton order
+        cz = (int)morton_compact(blockIdx.x);
+        cy = (int)morton_compact(blockIdx.x >> 1);
+        cx = (int)morton_compact(blockIdx.x >> 2);
+        if (cx >= n || cy >= n || cz >= n) return;
+    }
+    const int home = cell_id(cx, cy, cz, g);
     double pe_tot = 0.0, w_tot = 0.0;
     // ---- the 27 neighbour cells ("segments"): first slot, count, origin, exact origin offset
     int cnt = 0, start = 0;
@@ -183,7 +189,7 @@ k_fc3(const float4 *__restrict__ pos, const int *__restrict__ cell_start, const 
         oy = (ay == 0) ? 0.f : (ay > 0 ? ((cy == n - 1) ? g.last : g.side) : -((ny == n - 1) ? g.last : g.side));
         oz = (dz == 0) ? 0.f : (dz > 0 ? ((cz == n - 1) ? g.last : g.side) : -((nz == n - 1) ? g.last : g.side));
         ax_o = (float)nx * g.side; ay_o = (float)ny * g.side; az_o = (float)nz * g.side;
-        const int nb = (nx * n + ny) * n + nz;
+        const int nb = cell_id(nx, ny, nz, g);
         start = cell_start[nb];
         cnt = cell_start[nb + 1] - start;
     }
@@ -312,7 +318,7 @@ k_fc3(const float4 *__restrict__ pos, const int *__restrict__ cell_start, const 
                             const float qx = (dax == 0) ? 0.f : (dax > 0 ? ((cx == n - 1) ? g.last : g.side) : -((nx == n - 1) ? g.last : g.side));
                             const float qy = (day == 0) ? 0.f : (day > 0 ? ((cy == n - 1) ? g.last : g.side) : -((ny == n - 1) ? g.last : g.side));
                             const float qz = (ddz == 0) ? 0.f : (ddz > 0 ? ((cz == n - 1) ? g.last : g.side) : -((nz == n - 1) ? g.last : g.side));
-                            const float4 pj = pos[min(cell_start[(nx * n + ny) * n + nz] + kbeg + (rw >> 5), nmax)];
+                            const float4 pj = pos[min(cell_start[cell_id(nx, ny, nz, g)] + kbeg + (rw >> 5), nmax)];
                             ex = (((double)pj.x - (double)((float)nx * g.side)) + (double)qx) - ((double)pme.x - (double)hox);
                             ey = (((double)pj.y - (double)((float)ny * g.side)) + (double)qy) - ((double)pme.y - (double)hoy);
                             ez = (((double)pj.z - (double)((float)nz * g.side)) + (double)qz) - ((double)pme.z - (double)hoz);
@@ -378,7 +384,7 @@ k_fc3(const float4 *__restrict__ pos, const int *__restrict__ cell_start, const 
                     p.x = wrap_drift(fmaf(K.dt, v.x, p.x), g.L);
                     p.y = wrap_drift(fmaf(K.dt, v.y, p.y), g.L);
                     p.z = wrap_drift(fmaf(K.dt, v.z, p.z), g.L);
-                    const int c = (cell_coord(p.x, g) * n + cell_coord(p.y, g)) * n + cell_coord(p.z, g);
+                    const int c = cell_id(cell_coord(p.x, g), cell_coord(p.y, g), cell_coord(p.z, g), g);
                     v.w = __int_as_float(atomicAdd(&cell_count[c], 1));   // rank inside the new cell
                     pos_out[myslot] = p;
                     vel[myslot] = v;
@@ -401,8 +407,9 @@ k_fc3(const float4 *__restrict__ pos, const int *__restrict__ cell_start, const 
         pe_tot = warp_sum(pe_tot);
         w_tot = warp_sum(w_tot);
         if (lane == 0) {
-            part_pe[home] = 0.5 * pe_tot;                    // every pair is visited from both ends
-            part_w[home] = 0.5 * w_tot;
+            const int u = (cx * n + cy) * n + cz;            // partials by linear cell number in either ordering
+            part_pe[u] = 0.5 * pe_tot;                       // every pair is visited from both ends
+            part_w[u] = 0.5 * w_tot;
         }
     }
 }
@@ -412,7 +419,7 @@ k_fc3(const float4 *__restrict__ pos, const int *__restrict__ cell_start, const 
 int ljmd_forces_cell3(md_sim *s, bool energy, bool fused)
 {
     const Grid &g = s->grid;
-    const dim3 grid(g.n, g.n, g.n);
+    const dim3 grid = g.morton ? dim3((unsigned)g.nid, 1, 1) : dim3(g.n, g.n, g.n);
     if ((int64_t)g.ncells > s->part_cap) return MD_ENOMEM;
     double *ppe = s->part + (size_t)s->part_cap;
     double *pw = s->part + 2 * (size_t)s->part_cap;

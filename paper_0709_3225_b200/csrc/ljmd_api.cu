@@ -111,6 +111,7 @@ static void make_grid(const md_sim *s, double rc, Grid &g)
     if (n < 3) return;                               // g.n stays 0: cell path unavailable
     g.n = n;
     g.ncells = n * n * n;
+    g.nid = g.ncells;
     g.side = (float)side;
     g.last = (float)(L - (n - 1) * side);
     g.inv_side = (float)(1.0 / side);
@@ -281,6 +282,11 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->cell_of = (int *)ljmd_dev_alloc(N * sizeof(int), st);
     s->rank = (int *)ljmd_dev_alloc(N * sizeof(int), st);
     int ncells = s->grid.n ? s->grid.ncells : 1;
+    if (s->grid.n) {                                                   // room for the ids of the Morton numbering
+        int P = 1;
+        while (P < s->grid.n) P <<= 1;
+        if (P * P * P > ncells) ncells = P * P * P;
+    }
     s->cell_count = (int *)ljmd_dev_alloc((size_t)ncells * sizeof(int), st);
     s->cell_start = (int *)ljmd_dev_alloc(((size_t)ncells + 1) * sizeof(int), st);
     s->max_occ = (unsigned long long *)ljmd_dev_alloc(sizeof(unsigned long long), st);
@@ -782,10 +788,25 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
     } else if (!strcmp(key, "cell_group")) {
         if (value < 0 || value > 5) return MD_EINVAL;
         s->cell_group = (int)value;
+    } else if (!strcmp(key, "cell_order")) {
+        // 1 = cells numbered along a Morton curve (measurement; dense kernel only: it selects "cell_kernel" = 3)
+        if (value != 0 && value != 1) return MD_EINVAL;
+        s->grid.morton = (int)value;
+        s->grid.nid = s->grid.ncells;
+        if (s->grid.morton) {
+            int P = 1;
+            while (P < s->grid.n) P <<= 1;
+            s->grid.nid = P * P * P;
+            s->cell_kernel = 3;
+        }
+        s->layout = LAYOUT_NONE;
+        s->forces_valid = false;
+        CK(cudaMemsetAsync(s->cell_count, 0, (size_t)s->grid.nid * sizeof(int), s->stream));
     } else if (!strcmp(key, "fuse_integrator")) {
         s->fuse_integrator = value != 0.0;
     } else if (!strcmp(key, "cell_kernel")) {
         if (value != 1 && value != 2 && value != 3) return MD_EINVAL;
+        if (s->grid.morton && value != 3) return MD_EINVAL;          // the Morton numbering is the dense kernel's only
         s->cell_kernel = (int)value;
     } else if (!strcmp(key, "sort_every")) {
         if (value < 1) return MD_EINVAL;

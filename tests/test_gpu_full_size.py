@@ -82,10 +82,10 @@ def test_c4_cell_2048000(b, name):
     run_and_compare(b, name, 500, 1)
 
 
-@pytest.mark.parametrize("kernel,fuse", [(1, 0), (3, 0), (2, 1), (3, 1)])
-def test_c3_other_cell_kernels(b, kernel, fuse):
-    """The cell-force kernels that are not the default (the first ballot kernel, the dense kernel, and the
-    integrator fused into the force epilogue) on the full config-3 system, every atom."""
+@pytest.mark.parametrize("kernel,fuse,morton", [(1, 0, 0), (3, 0, 0), (2, 1, 0), (3, 1, 0), (3, 0, 1), (3, 1, 1)])
+def test_c3_other_cell_kernels(b, kernel, fuse, morton):
+    """The cell-force kernels that are not the default (the first ballot kernel, the dense kernel, the
+    integrator fused into the force epilogue, Morton cell numbering) on the full config-3 system, every atom."""
     sysd = wl.md_system("c3_cell_256k", velocities_from(gpu_uniforms(b)))
     N, L = sysd["N"], sysd["L"]
     import os
@@ -93,6 +93,10 @@ def test_c3_other_cell_kernels(b, kernel, fuse):
     with b.Sim(N, L) as s:
         s.option("cell_kernel", kernel)
         s.option("fuse_integrator", fuse)
+        if morton:
+            s.option("cell_order", 1)                      # cells numbered along a Morton curve (dense kernel)
+            with pytest.raises(b.MDError):
+                s.option("cell_kernel", 2)
         s.set_state(sysd["pos"], sysd["vel"])
         s.step(300, 1)
         ke, pe, w = s.energies()
