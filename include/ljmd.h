@@ -163,6 +163,8 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
  *   "cell_skin"      MD_CELL on skin cells: cells of side >= rc + value, re-sorted on the device's own
  *                    decision when an atom has strayed value / 2; 0 (default) = the cell
  *                    list is rebuilt every step.  Shares the skin with MD_VERLET (set before either runs)
+ *   "vl_fuse"        1 (default): interior steps of md_step(MD_VERLET) integrate in the epilogue of the list
+ *                    force kernel (full lists only); 0 = separate integration kernel
  *   "vl_half"        MD_VERLET with half lists: every pair once, the reaction force through vector
  *                    reductions (default 0; measured in DESIGN.md section 7b)
  *   "cell_group"     cells of one z-column handled by one warp of the cell-force kernel (1..5);

@@ -51,7 +51,7 @@ struct Grid {
 struct GraphEntry {
     cudaGraphExec_t exec;
     int algo, unit, since_sort, layout, stamp;
-    void *pos, *vel;
+    void *pos, *vel, *lpos;
     int64_t launches;             // kernels per replay
     cudaStream_t stream;
 };
@@ -92,6 +92,7 @@ struct md_sim {
     float4 *vl_lbuild;    // [N] local coordinates at the last build
     VlCtl *vl_ctl;
     int vl_cap, vl_npad;
+    bool vl_fuse;         // option "vl_fuse": interior steps of md_step(MD_VERLET) integrate in the force kernel's epilogue
     bool vl_half;         // option "vl_half": half lists + vector reductions for the reactions (measurement)
     bool vl_naive_build;  // option "vl_naive_build": thread-per-atom list kernel instead of the warp filter
     int grid_paper_n;     // int[L/rc]
@@ -101,6 +102,7 @@ struct md_sim {
     float4 *pos, *vel, *frc;
     float4 *pos2, *vel2;          // scatter targets (cell build)
     float4 *lpos;                 // cell-local coordinates in slot order (after a build)
+    float4 *lpos2;                // list path with the fused integrator: the local coordinates of the next step
     int *cell_of;                 // [N] cell id per slot (after a build)
     int *rank;                    // [N] rank inside its cell (during a build)
     int *cell_count;              // [ncells]
@@ -183,7 +185,7 @@ int ljmd_kick_andersen(md_sim *s);                   // rand48.cu: second half-k
 int ljmd_mb_velocities(md_sim *s, double T, uint64_t seed48, double *vraw, double *part, double *mom);   // rand48.cu
 int ljmd_vl_kick_drift(md_sim *s, int kicks);
 int ljmd_vl_build_lists(md_sim *s, const int *cond);    // force_cell.cu: lists through the cell kernel's filter
-int ljmd_forces_verlet(md_sim *s);
+int ljmd_forces_verlet(md_sim *s, bool fuse = false);   // fuse: the epilogue integrates (full lists)
 int ljmd_vl_stats(md_sim *s, int *nbuilds, int *nsteps, int *overflow);
 int ljmd_vl_grow(md_sim *s, int need);               // longer lists after an overflow; the next evaluation rebuilds
 int ljmd_cell_build(md_sim *s);

@@ -215,7 +215,7 @@ static void free_all(md_sim *s)
     for (int k = 0; k < s->ev_cap; k++) cudaEventDestroy(s->ev_pool[k]);
     free(s->ev_pool);
     free(s->ev_tag);
-    void *ptrs[] = {s->pos, s->vel, s->frc, s->pos2, s->vel2, s->lpos, s->cell_of, s->rank, s->cell_count,
+    void *ptrs[] = {s->pos, s->vel, s->frc, s->pos2, s->vel2, s->lpos, s->lpos2, s->cell_of, s->rank, s->cell_count,
                     s->cell_start, s->max_occ, s->scan_ctl, s->scan_state, s->vl_list, s->vl_count, s->vl_lbuild, s->vl_ctl, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list, s->and_t_dev,
                     s->tile_start};
     for (void *p : ptrs) ljmd_dev_free(p, st);
@@ -251,6 +251,7 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->sort_every = 10;
     s->skin = 0.3 * sigma;
     s->cell_kernel = 2;
+    s->vl_fuse = true;
     setup_grid(s);
     setup_pair(s);
 
@@ -488,7 +489,7 @@ static int eval_forces(md_sim *s, int algo, bool energy = true, bool fuse = fals
 {
     int r;
     if (algo == MD_VERLET) {
-        if ((r = ljmd_forces_verlet(s))) return r;
+        if ((r = ljmd_forces_verlet(s, fuse))) return r;
     } else if (algo == MD_CELL && s->cell_skin_on) {
         if ((r = ljmd_forces_skincell(s, energy))) return r;
     } else if (algo == MD_CELL && s->cell_kernel >= 2) {
@@ -514,14 +515,15 @@ static int one_step(md_sim *s, int algo, int kicks, bool last, bool energy, bool
     int r;
     const bool skinc = algo == MD_CELL && s->cell_skin_on;        // slots are stable between re-sorts: the list path's integrator
     const bool k3 = algo == MD_CELL && s->cell_kernel >= 2 && !skinc;      // lean build, fusable force kernel
-    if (!(k3 && s->fused_pending)) {                   // else: the previous force kernel has integrated already
+    const bool vfu = algo == MD_VERLET && s->vl_fuse && !s->vl_half;
+    if (!((k3 || vfu) && s->fused_pending)) {          // else: the previous force kernel has integrated already
         if ((r = skinc ? ljmd_vl_kick_drift(s, kicks)
                  : (algo == MD_CELL) ? (k3 ? ljmd_kick_drift_bin3(s, kicks) : ljmd_kick_drift_bin(s, kicks))
                                    : (algo == MD_VERLET) ? ljmd_vl_kick_drift(s, kicks) : ljmd_kick_drift(s, kicks)))
             return r;
         ljmd_tick(s, TAG_INTEGRATE);
     }
-    if ((r = eval_forces(s, algo, energy, k3 && !last && may_fuse && s->fuse_integrator))) return r;
+    if ((r = eval_forces(s, algo, energy, !last && may_fuse && ((k3 && s->fuse_integrator) || vfu)))) return r;
     if (last) {
         if ((r = ljmd_kick_ke(s))) return r;
         ljmd_tick(s, TAG_INTEGRATE);
@@ -547,7 +549,7 @@ static int graph_unit(const md_sim *s, int algo)
 {
     if (algo == MD_CELL && s->cell_skin_on) return 1;
     if (algo == MD_CELL) return 2;
-    if (algo == MD_VERLET) return 1;                  // no buffer swaps: builds are decided and done on the device
+    if (algo == MD_VERLET) return (s->vl_fuse && !s->vl_half) ? 2 : 1;   // no buffer swaps but the fused integrator's (builds are decided and done on the device)
     if (s->ap_tiled && !s->ap_force_general) return 2 * s->sort_every;
     return 1;
 }
@@ -572,6 +574,7 @@ static int replay_interior(md_sim *s, int algo, int unit, int64_t nunits, int64_
     for (int i = 0; i < MD_NGRAPH; i++) {
         GraphEntry &e = s->graphs[i];
         if (e.exec && e.algo == algo && e.unit == unit && e.pos == (void *)s->pos && e.vel == (void *)s->vel &&
+            e.lpos == (void *)s->lpos &&
             e.since_sort == s->ap_since_sort && e.layout == s->layout && e.stream == run)
             g = &e;
     }
@@ -583,7 +586,7 @@ static int replay_interior(md_sim *s, int algo, int unit, int64_t nunits, int64_
             if (s->graphs[i].stamp < s->graphs[victim].stamp) victim = i;
         GraphEntry e;
         memset(&e, 0, sizeof(e));
-        e.algo = algo; e.unit = unit; e.pos = s->pos; e.vel = s->vel; e.since_sort = s->ap_since_sort;
+        e.algo = algo; e.unit = unit; e.pos = s->pos; e.vel = s->vel; e.lpos = s->lpos; e.since_sort = s->ap_since_sort;
         e.layout = s->layout; e.stream = run;
         const md_sim saved = *s;                        // plain data: restored if the capture fails
         const int64_t l0 = s->launches;
@@ -598,7 +601,7 @@ static int replay_interior(md_sim *s, int algo, int unit, int64_t nunits, int64_
         }
         if (r == MD_OK && cudaGraphInstantiate(&e.exec, graph, 0) != cudaSuccess) r = MD_ECUDA;
         if (graph) cudaGraphDestroy(graph);
-        const bool same = s->pos == saved.pos && s->vel == saved.vel && s->ap_since_sort == saved.ap_since_sort &&
+        const bool same = s->pos == saved.pos && s->vel == saved.vel && s->lpos == saved.lpos && s->ap_since_sort == saved.ap_since_sort &&
                           s->layout == saved.layout;
         e.launches = s->launches - l0;
         s->stream = user;
@@ -765,6 +768,8 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
         s->and_thr = (s->and_T > 0) ? (uint32_t)thr : 0u;
         s->and_t = 0;                                                 // the stream starts over
         CK(cudaMemsetAsync(s->and_t_dev, 0, sizeof(uint64_t), s->stream));
+    } else if (!strcmp(key, "vl_fuse")) {
+        s->vl_fuse = value != 0.0;
     } else if (!strcmp(key, "vl_half")) {
         s->vl_half = value != 0.0;
         s->layout = LAYOUT_NONE;                        // rebuild the lists in the other form

@@ -253,11 +253,23 @@ __device__ __forceinline__ void vl_react(float4 *frc, int j, float x, float y, f
 // HALF (option "vl_half", a measurement of Newton's third law on this path): the lists hold
 // every pair once; the force on i is summed in registers and added to frc[i] at the end, the reaction goes to
 // frc[j] pair by pair through red.global.add.v4.f32; frc is zeroed before the launch.
-template <bool MODE2, bool HALF>
+// Fused integrator of the list path (option "vl_fuse"): what the epilogue of k_vl_force<.., FUSED> needs.
+struct VlFuse {
+    float4 *pos, *vel, *lnext;        // lnext: the local coordinates of the next step (the others read lpos meanwhile)
+    const float4 *lbuild;
+    VlCtl *ctl;
+    float hdt, dt;
+};
+
+// FUSED (full lists only): the thread that owns F_i applies the closing half-kick of this step and the opening
+// half-kick, drift, wrap, local coordinate and displacement check of the next one (the arithmetic of
+// k_vl_kick_drift<2>): slots are stable between rebuilds, so an interior step is this one kernel plus the
+// conditional build launches.
+template <bool MODE2, bool HALF, bool FUSED>
 __global__ void __launch_bounds__(VL_T, VL_MINB)
 k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams P, VlConst K,
            const unsigned *__restrict__ list, const int *__restrict__ count, float4 *__restrict__ frc,
-           double *__restrict__ part_pe, double *__restrict__ part_w)
+           double *__restrict__ part_pe, double *__restrict__ part_w, VlFuse U)
 {
     __shared__ float4 offt[128];
     __shared__ unsigned queue[VL_Q][VL_T];
@@ -267,6 +279,7 @@ k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams 
     __syncthreads();
     const int i = blockIdx.x * VL_T + threadIdx.x;
     double pe = 0.0, w = 0.0;
+    float d2move = 0.f;
     if (i < N) {
         const float4 li = lpos[i];
         const int cnt = count[i];
@@ -342,14 +355,48 @@ k_vl_force(const float4 *__restrict__ lpos, int N, int npad, Grid g, PairParams 
                 }
             }
         }
-        if (HALF) vl_react(frc, i, (float)(dfx + (double)fx), (float)(dfy + (double)fy), (float)(dfz + (double)fz));
-        else frc[i] = make_float4((float)(dfx + (double)fx), (float)(dfy + (double)fy), (float)(dfz + (double)fz), 0.f);
+        const float Fx = (float)(dfx + (double)fx), Fy = (float)(dfy + (double)fy), Fz = (float)(dfz + (double)fz);
+        if (HALF) vl_react(frc, i, Fx, Fy, Fz);
+        else if (!FUSED) frc[i] = make_float4(Fx, Fy, Fz, 0.f);
+        else {
+            float4 p = U.pos[i], v = U.vel[i];
+#pragma unroll
+            for (int k = 0; k < 2; k++) {
+                v.x = fmaf(U.hdt, Fx, v.x);
+                v.y = fmaf(U.hdt, Fy, v.y);
+                v.z = fmaf(U.hdt, Fz, v.z);
+            }
+            p.x = wrap_drift(fmaf(U.dt, v.x, p.x), g.L);
+            p.y = wrap_drift(fmaf(U.dt, v.y, p.y), g.L);
+            p.z = wrap_drift(fmaf(U.dt, v.z, p.z), g.L);
+            const int c = __float_as_int(li.w) & VL_CELLMASK;
+            const int cz = c % g.n, cy = (c / g.n) % g.n, cx = c / (g.n * g.n);
+            float4 l;
+            l.x = vl_local(p.x, cx, g);
+            l.y = vl_local(p.y, cy, g);
+            l.z = vl_local(p.z, cz, g);
+            l.w = li.w;
+            U.pos[i] = p;
+            U.vel[i] = v;
+            U.lnext[i] = l;
+            const float4 l0 = U.lbuild[i];
+            const float ex = l.x - l0.x, ey = l.y - l0.y, ez = l.z - l0.z;
+            d2move = fmaf(ex, ex, fmaf(ey, ey, ez * ez));
+        }
         pe = dpe + P.eps4 * ((double)sA - (double)sB) - (double)nin * P.ushift;
         w = dw + P.eps24 * (2.0 * (double)sA - (double)sB);
         if (MODE2) {
             pe += P.f_rc * (double)sR;
             w -= P.f_rc * ((double)sR + (double)nin * P.rc);
         }
+    }
+    if (FUSED) {
+        d2move = fmaxf(d2move, __shfl_xor_sync(0xffffffffu, d2move, 16));
+        d2move = fmaxf(d2move, __shfl_xor_sync(0xffffffffu, d2move, 8));
+        d2move = fmaxf(d2move, __shfl_xor_sync(0xffffffffu, d2move, 4));
+        d2move = fmaxf(d2move, __shfl_xor_sync(0xffffffffu, d2move, 2));
+        d2move = fmaxf(d2move, __shfl_xor_sync(0xffffffffu, d2move, 1));
+        if ((threadIdx.x & 31) == 0 && d2move > 0.f) atomicMax(&U.ctl->maxd2, __float_as_uint(d2move));
     }
     pe = block_sum(pe, red);
     w = block_sum(w, red);
@@ -367,9 +414,10 @@ static int vl_alloc_base(md_sim *s)
     if (s->vl_ctl) return MD_OK;
     s->vl_lbuild = (float4 *)ljmd_dev_alloc((size_t)s->N * sizeof(float4), s->stream);
     s->vl_ctl = (VlCtl *)ljmd_dev_alloc(sizeof(VlCtl), s->stream);
-    if (!s->vl_lbuild || !s->vl_ctl) {
-        ljmd_dev_free(s->vl_lbuild, s->stream); ljmd_dev_free(s->vl_ctl, s->stream);
-        s->vl_lbuild = nullptr; s->vl_ctl = nullptr;
+    s->lpos2 = (float4 *)ljmd_dev_alloc((size_t)s->N * sizeof(float4), s->stream);
+    if (!s->vl_lbuild || !s->vl_ctl || !s->lpos2) {
+        ljmd_dev_free(s->vl_lbuild, s->stream); ljmd_dev_free(s->vl_ctl, s->stream); ljmd_dev_free(s->lpos2, s->stream);
+        s->vl_lbuild = nullptr; s->vl_ctl = nullptr; s->lpos2 = nullptr;
         return MD_ENOMEM;
     }
     CK(cudaMemsetAsync(s->vl_ctl, 0, sizeof(VlCtl), s->stream));
@@ -483,10 +531,12 @@ int ljmd_forces_skincell(md_sim *s, bool energy)
 }
 
 // Decide, (re)build if the device-side flag says so, evaluate forces from the lists.
-int ljmd_forces_verlet(md_sim *s)
+int ljmd_forces_verlet(md_sim *s, bool fuse)
 {
     int r = vl_alloc(s);
     if (r) return r;
+    s->fused_pending = false;
+    fuse = fuse && !s->vl_half;
     const int N = (int)s->N, nbl = (N + VL_T - 1) / VL_T;
     const Grid &g = s->vgrid;
     if ((r = vl_decide_and_sort(s, LAYOUT_VERLET))) return r;
@@ -513,19 +563,29 @@ int ljmd_forces_verlet(md_sim *s)
         // (30 % still holds eight blocks' tables and queues); measured 3 % faster than the default split
         static bool carved = false;
         if (!carved) {
-            cudaFuncSetAttribute(k_vl_force<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
-            cudaFuncSetAttribute(k_vl_force<true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
-            cudaFuncSetAttribute(k_vl_force<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
-            cudaFuncSetAttribute(k_vl_force<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
+            cudaFuncSetAttribute(k_vl_force<false, false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
+            cudaFuncSetAttribute(k_vl_force<true, false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
+            cudaFuncSetAttribute(k_vl_force<false, true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
+            cudaFuncSetAttribute(k_vl_force<true, true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
+            cudaFuncSetAttribute(k_vl_force<false, false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
+            cudaFuncSetAttribute(k_vl_force<true, false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 30);
             carved = true;
         }
     }
     if (s->vl_half) CK(cudaMemsetAsync(s->frc, 0, (size_t)N * sizeof(float4), s->stream));
-#define VL_LAUNCH(M2, H) \
-    k_vl_force<M2, H><<<nbl, VL_T, 0, s->stream>>>(s->lpos, N, s->vl_npad, g, P, K, s->vl_list, s->vl_count, s->frc, ppe, pw)
-    if (P.mode == 2) { if (s->vl_half) VL_LAUNCH(true, true); else VL_LAUNCH(true, false); }
-    else { if (s->vl_half) VL_LAUNCH(false, true); else VL_LAUNCH(false, false); }
+    VlFuse U;
+    U.pos = s->pos; U.vel = s->vel; U.lnext = s->lpos2; U.lbuild = s->vl_lbuild; U.ctl = s->vl_ctl;
+    U.hdt = s->hdtf; U.dt = s->dtf;
+#define VL_LAUNCH(M2, H, F) \
+    k_vl_force<M2, H, F><<<nbl, VL_T, 0, s->stream>>>(s->lpos, N, s->vl_npad, g, P, K, s->vl_list, s->vl_count, s->frc, ppe, pw, U)
+    if (fuse) { if (P.mode == 2) VL_LAUNCH(true, false, true); else VL_LAUNCH(false, false, true); }
+    else if (P.mode == 2) { if (s->vl_half) VL_LAUNCH(true, true, false); else VL_LAUNCH(true, false, false); }
+    else { if (s->vl_half) VL_LAUNCH(false, true, false); else VL_LAUNCH(false, false, false); }
 #undef VL_LAUNCH
+    if (fuse) {                                          // the next step reads what this epilogue wrote
+        float4 *t = s->lpos; s->lpos = s->lpos2; s->lpos2 = t;
+        s->fused_pending = true;
+    }
     CKL(s);
     ljmd_tick(s, TAG_FORCE);
     s->n_pe = nbl;

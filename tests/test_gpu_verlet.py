@@ -234,3 +234,26 @@ def test_half_lists_full_size_c3(b):
     Fo, peo, wo = oracle.forces(p.astype(np.float64), sysd["L"], algo=1)
     check_forces(F, Fo, p, sysd["L"], oracle)
     assert pe == pytest.approx(peo, rel=1e-6) and w == pytest.approx(wo, rel=1e-6)
+
+
+@pytest.mark.parametrize("fuse", [1, 0])
+@pytest.mark.parametrize("graph,chunks", [(1, [100]), (0, [100]), (1, [7, 1, 30, 2, 60])])
+def test_fused_integrator_of_the_list_path(b, c1, fuse, graph, chunks):
+    """Option "vl_fuse" (default 1): interior steps integrate in the epilogue of the list force kernel (slots are
+    stable between rebuilds: one kernel per step plus the conditional build launches).  Same energies as the oracle
+    after 100 steps however the steps are split over calls, graph-replayed or not, fused or not."""
+    _, _, _, tr = oracle.verlet_run(c1["pos"], c1["vel"], c1["L"], 100, algo=0)
+    with b.Sim(c1["N"], c1["L"]) as s:
+        s.option("vl_fuse", fuse)
+        s.option("graph", graph)
+        s.set_state(c1["pos"], c1["vel"])
+        for k in chunks:
+            s.step(k, b.MD_VERLET)
+        ke, pe, w = s.energies()
+        Eo = tr[100, 0] + tr[100, 1]
+        assert abs(ke + pe - Eo) <= 1e-5 * abs(Eo)
+        p, v = s.get_state()
+        Fo, _, _ = oracle.forces(p.astype(np.float64), c1["L"], algo=0)
+        assert force_check(s.forces(), Fo)[0] == 0
+        assert s.stat("vl_steps") == 101 and 3 <= s.stat("vl_builds") <= 40
+        assert ke == pytest.approx(oracle.kinetic_energy(v.astype(np.float64)), rel=1e-9)
