@@ -130,6 +130,34 @@ int md_set_stream(md_sim *s, void *cuda_stream);
  * Marks the forces stale.  MD_EINVAL for an unknown kind, non-finite a or b, or b < 0. */
 int md_set_potential(md_sim *s, int kind, double a, double b);
 
+/* All-pairs forces, PE and virial WITHOUT any device allocation: for callers that cannot call cudaMalloc.
+ * That is a process whose memory pool took the whole card at start-up (a cudaMalloc made by a library then
+ * fails), or a loop with a latency budget, where cudaMalloc / cudaFree are ruled out because they stall the
+ * whole device.  md_create and the calls on a handle do allocate; this one call never does.
+ *
+ * Computes what md_compute_forces(MD_ALLPAIRS) computes (Eq. 1, with the Lennard-Jones pair
+ * of PAPER.md:56-61 and the same meaning of rc, eps, sigma, shifted as md_create; every in-range pair in
+ * FP64; box (double)(float)L, minimum image): forces[i] = F_i, pe_virial[0] = sum_{i<j} U,
+ * pe_virial[1] = sum_{i<j} r f.  Stateless: no handle, no velocities, Lennard-Jones only.
+ *   pos        [N][3] floats, DEVICE memory, read only, expected in [0, L) (used as given, not wrapped)
+ *   forces     [N][3] floats, DEVICE memory, overwritten, same atom order as pos
+ *   pe_virial  2 doubles,     DEVICE memory, overwritten
+ * All three stay the caller's; host pointers are refused (MD_EINVAL), since staging them would need an
+ * allocation.  Runs on cuda_stream (a cudaStream_t; NULL = legacy default stream) and returns after that
+ * stream has finished the work, like every other call here.
+ *
+ * Scratch: the partial sums of the kernel live in one array built into the library, about 1.3 MB, which each
+ * GPU that loads the library keeps until the process exits.  Its fixed size sets the limit
+ * N <= MD_STATIC_MAX_ATOMS; a larger N returns MD_EUNSUPPORTED and nothing is launched.  Every call on a
+ * device shares that array (it keeps the previous call's contents; what must start at zero is cleared by each
+ * call itself), so calls that overlap on the GPU -- two host threads, two streams -- race with each other:
+ * serialise them.  The first call on each device looks up the array's device address
+ * (cudaGetSymbolAddress, with that device current); make that first call before starting any stream capture.
+ * Errors: MD_EINVAL as md_create, plus NULL or non-device pointers; MD_EUNSUPPORTED; MD_ECUDA. */
+#define MD_STATIC_MAX_ATOMS 16384
+int md_forces_allpairs_static(const float *pos, int64_t N, double L, double rc, double eps, double sigma,
+                              int shifted, float *forces, double *pe_virial, void *cuda_stream);
+
 /* The same on an explicit CUDA stream (no process-wide state involved). */
 int rand48_fill_on(uint64_t *seeds, int64_t nstreams, int64_t ndraws, int kind, void *out, void *cuda_stream);
 

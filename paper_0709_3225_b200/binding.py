@@ -24,6 +24,7 @@ MD_ALLPAIRS, MD_CELL, MD_VERLET = 0, 1, 2
 MD_TRUNCATED, MD_ENERGY_SHIFTED, MD_FORCE_SHIFTED = 0, 1, 2
 MD_POT_LJ, MD_POT_YUKAWA = 0, 1
 R48_U32_HI32, R48_U32_HI31, R48_F64, R48_U64_STATE = 0, 1, 2, 3
+MD_STATIC_MAX_ATOMS = 16384        # include/ljmd.h; tests/test_abi.py keeps the two equal
 R48_DTYPES = {0: np.uint32, 1: np.uint32, 2: np.float64, 3: np.uint64}
 
 _vp, _i64, _i32, _d = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double
@@ -52,6 +53,7 @@ _SIGS = {
     "md_get_stat": ([_vp, ctypes.c_char_p, _pd], _i32),
     "md_last_cuda_error": ([], ctypes.c_char_p),
     "rand48_kernel_launches": ([], _i64),
+    "md_forces_allpairs_static": ([_vp, _i64, _d, _d, _d, _d, _i32, _vp, _vp, _vp], _i32),
 }
 for _name, (_args, _res) in _SIGS.items():
     _fn = getattr(_lib, _name)          # AttributeError here = header/library mismatch
@@ -191,6 +193,22 @@ def md_get_stat(h, key):
 
 def rand48_kernel_launches():
     return _lib.rand48_kernel_launches()
+
+
+def md_forces_allpairs_static(pos, N, L, rc, eps, sigma, shifted, forces, pe_virial, stream=None):
+    """md_forces_allpairs_static: all-pairs forces, PE and virial for callers that cannot allocate device memory
+    (their own pool owns the whole card, or cudaMalloc's device-wide stall is not allowed where they run).
+    pos [N,3] float32, forces [N,3] float32 and pe_virial [2] float64 must all be DEVICE arrays of the
+    caller; the library's scratch is a fixed 1.3 MB array inside the .so, hence N <= MD_STATIC_MAX_ATOMS.
+    Calls share that array: do not let two of them overlap on the GPU.  Runs on `stream` (default:
+    PyTorch's current stream) and returns when the results are complete."""
+    if N > MD_STATIC_MAX_ATOMS:
+        raise MDError(MD_EUNSUPPORTED, "md_forces_allpairs_static: N = %d exceeds MD_STATIC_MAX_ATOMS = %d, "
+                      "the size its built-in scratch array is made for (use md_create + md_compute_forces)"
+                      % (N, MD_STATIC_MAX_ATOMS))
+    st = current_stream() if stream is None else int(stream)
+    _check(_lib.md_forces_allpairs_static(_addr(pos), N, L, rc, eps, sigma, shifted, _addr(forces), _addr(pe_virial),
+                                          st), "md_forces_allpairs_static")
 
 
 def use_torch_allocator():
