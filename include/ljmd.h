@@ -10,7 +10,9 @@
  *   - Every array pointer is owned by the caller, may be HOST or DEVICE memory (detected
  *     with cudaPointerGetAttributes), and is not retained after the call returns.
  *   - Calls are synchronous for the caller: results are complete on return.  Kernels run
- *     on the stream set with md_set_stream (default: the legacy default stream).
+ *     on the stream set with md_set_stream (default: the legacy default stream; the Python
+ *     binding's md_create sets PyTorch's current stream and allocator instead, unless it is
+ *     called with torch_plumbing=False).
  *   - A handle is not thread-safe; distinct handles are independent.
  *   - Everything executes on the current CUDA device in sm_100a kernels.  There is no CPU
  *     fallback: without a usable device every call returns MD_ECUDA.
@@ -205,22 +207,37 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
  *                    (1.5 sigma^2 when the cell kernel groups several cells per warp); 0 = FP32 for
  *                    every pair but the sliver around rc^2; a huge value = FP64 for every in-range
  *                    pair.  The all-pairs path always evaluates every in-range pair in FP64.
+ *                    Lennard-Jones only: MD_EINVAL while another potential is set (the FP32 branch is
+ *                    Lennard-Jones arithmetic; md_set_potential keeps every pair in FP64)
  *   "cell_kernel"    cell-force kernel: 2 (default) ballot filter + per-lane walk (force_cell2.cu),
  *                    1 its first version (force_cell.cu), 3 dense evaluation of every staged
  *                    candidate (force_cell3.cu); same forces within the tolerances of DESIGN.md 12
  *   "cell_order"     1 = cells numbered along a Morton curve instead of linearly (dense kernel only: selects
- *                    "cell_kernel" = 3; default 0: measured slower)
+ *                    "cell_kernel" = 3; default 0: measured slower).  Kept across later
+ *                    "skin" / "cell_skin" options.  The cell arrays are sized for n^3 ids at md_create and
+ *                    enlarged to the padded cube (up to 8 n^3) only here: MD_ENOMEM if that fails,
+ *                    MD_EDOMAIN without a cell grid
  *   "fuse_integrator" 1 = interior steps of md_step(MD_CELL) integrate in the force kernel's epilogue
  *                    (kernels 2 and 3; default 0: measured slower)
  *   "sort_every"     all-pairs path: re-sort atoms along the Hilbert curve every k steps (default 10)
  *   "ap_general"     1 = force the unsorted per-pair-minimum-image all-pairs kernel
  *   "ap_R"           atoms per thread (1, 2, 4, 8) of the sorted all-pairs kernel, overriding the
  *                    choice made from N and L; blocks too wide for the box test per-pair images
- * md_get_stat keys: "ncell" (cells per dimension), "max_occupancy", "kernel_launches"
- * (kernels launched by this handle so far, graph nodes included), "graph_replays", "vl_builds", "vl_steps",
- * "vl_overflow", "vl_cap" (neighbour-list builds, evaluations, 0 or the list length the last build needed
- * beyond the capacity, capacity), "steps_done",
- * "side" (cell side). */
+ *   "vl_naive_build" 1 = MD_VERLET lists built by the thread-per-atom kernel instead of the cell kernel's warp
+ *                    filter (default 0; the cross-check of the two builders)
+ * Any other key is MD_EINVAL.  Limits: N <= 2^30 (md_create: MD_EINVAL beyond), N <= 2^23 - 1 for MD_VERLET,
+ * at most 1023 cells per dimension (a larger box gets wider cells).
+ * md_get_stat keys: "ncell" (cells per dimension), "side" (cell side), "last_side" (width of the last cell of a
+ * row, >= side: it takes the remainder of L), "cell_order", "cell_ids" (numbering in force and how many ids it
+ * spans), "max_occupancy", "kernel_launches" (kernels launched by this handle so far, graph nodes included),
+ * "graph_replays", "steps_done", "precise_r2" (the window in force),
+ * "vl_builds", "vl_steps", "vl_cap", "vl_overflow" (neighbour-list builds, evaluations, capacity, and 0 or the
+ * longest list any build since the last host-requested one needed beyond the capacity: sticky, so a list
+ * truncated in the middle of md_step is reported at its end even if later builds fitted),
+ * "ap_tiled", "ap_R", "ap_ntiles", "ap_tsplit", "ap_nsplit" (all-pairs launch shape: sorted kernel in use, atoms
+ * per thread, i blocks, j splits; j splits of the general kernel), "nbr_cap" (candidate-list capacity per atom of
+ * the sorted all-pairs kernel, 0 before its first use), "andersen_threshold", "andersen_steps",
+ * "t_integrate_ms", "t_build_ms", "t_force_ms", "t_force2_ms", "t_other_ms", "n_force" (with "time_kernels"). */
 int md_set_option(md_sim *s, const char *key, double value);
 int md_get_stat(md_sim *s, const char *key, double *value);
 

@@ -146,6 +146,8 @@ struct md_sim {
     bool precise_r2_user;         // "precise_r2" was set through md_set_option
     int cell_group;               // cells per row group of the cell-force kernel; 0 = automatic
     int cell_kernel;              // 2 (default): force_cell2.cu; 3: force_cell3.cu (dense); 1: force_cell.cu
+    int cell_order;               // option "cell_order" (1 = Morton numbering); re-applied to `grid` whenever it is rebuilt
+    int cell_cap;                 // ints allocated for cell_count (cell_start has one more)
     bool cell_skin_on;            // option "cell_skin" > 0: MD_CELL runs on skin cells (verlet.cu)
     bool fuse_integrator;         // option "fuse_integrator": interior steps integrate in the force kernel's epilogue
     int64_t launches, steps_done;
@@ -168,6 +170,7 @@ enum { LAYOUT_NONE = 0, LAYOUT_CELL = 1, LAYOUT_TILE = 2, LAYOUT_VERLET = 3, LAY
 // Record an event; the time since the previous tick is attributed to `tag`.
 void ljmd_tick(md_sim *s, int tag);
 int ljmd_collect_ticks(md_sim *s);
+void ljmd_drop_graphs(md_sim *s);                   // ljmd_api.cu: forget every cached CUDA graph of the handle
 
 // ---- kernels' host launchers (each returns md_status) ---------------------------
 int ljmd_pack_state(md_sim *s, const float *dpos, const float *dvel);

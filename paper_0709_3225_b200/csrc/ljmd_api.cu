@@ -117,12 +117,26 @@ static void make_grid(const md_sim *s, double rc, Grid &g)
     g.inv_side = (float)(1.0 / side);
 }
 
+// Number of cell ids of the Morton numbering: the padded cube P^3, P the power of two >= n.
+static int morton_ids(int n)
+{
+    int P = 1;
+    while (P < n) P <<= 1;
+    return P * P * P;
+}
+
 static void setup_grid(md_sim *s)
 {
     s->grid_paper_n = (int)floor(s->L / s->rc);
     make_grid(s, s->rc, s->grid);
     make_grid(s, s->rc + s->skin + 1e-3, s->vgrid);  // neighbour-list path: cells wider than rc + skin (margin: see
                                                      // the list mode of force_cell.cu)
+    // make_grid starts from a cleared Grid: the numbering chosen with "cell_order" is put back, so that a later
+    // "skin" or "cell_skin" does not silently return the cells to the linear numbering
+    if (s->cell_order && s->grid.n) {
+        s->grid.morton = 1;
+        s->grid.nid = morton_ids(s->grid.n);
+    }
 }
 
 static void setup_pair(md_sim *s)
@@ -198,7 +212,9 @@ int ljmd_collect_ticks(md_sim *s)
 }
 
 // ---- create / destroy -----------------------------------------------------------------
-static void drop_graphs(md_sim *s)
+// Every cached graph has buffer addresses and capacities baked into its nodes: whoever reallocates a buffer a
+// captured kernel uses (ljmd_vl_grow) or changes what the kernels are launched with calls this.
+void ljmd_drop_graphs(md_sim *s)
 {
     for (int k = 0; k < MD_NGRAPH; k++) {
         if (s->graphs[k].exec) cudaGraphExecDestroy(s->graphs[k].exec);
@@ -282,12 +298,9 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->lpos = (float4 *)ljmd_dev_alloc(f4, st);
     s->cell_of = (int *)ljmd_dev_alloc(N * sizeof(int), st);
     s->rank = (int *)ljmd_dev_alloc(N * sizeof(int), st);
+    // n^3 cells; the padded cube of the Morton numbering is allocated when "cell_order" asks for it
     int ncells = s->grid.n ? s->grid.ncells : 1;
-    if (s->grid.n) {                                                   // room for the ids of the Morton numbering
-        int P = 1;
-        while (P < s->grid.n) P <<= 1;
-        if (P * P * P > ncells) ncells = P * P * P;
-    }
+    s->cell_cap = ncells;
     s->cell_count = (int *)ljmd_dev_alloc((size_t)ncells * sizeof(int), st);
     s->cell_start = (int *)ljmd_dev_alloc(((size_t)ncells + 1) * sizeof(int), st);
     s->max_occ = (unsigned long long *)ljmd_dev_alloc(sizeof(unsigned long long), st);
@@ -358,7 +371,7 @@ extern "C" int md_set_potential(md_sim *s, int kind, double a, double b)
     else if (was_yukawa) s->precise_r2_user = false;
     setup_pair(s);
     s->forces_valid = false;
-    drop_graphs(s);
+    ljmd_drop_graphs(s);
     return MD_OK;
 }
 
@@ -367,7 +380,7 @@ extern "C" int md_set_stream(md_sim *s, void *stream)
     if (!s) return MD_EINVAL;
     CK(cudaStreamSynchronize(s->stream));
     s->stream = (cudaStream_t)stream;
-    drop_graphs(s);
+    ljmd_drop_graphs(s);
     return MD_OK;
 }
 
@@ -740,6 +753,9 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
     }
     else if (!strcmp(key, "precise_r2")) {
         if (!(value >= 0)) return MD_EINVAL;
+        // the FP32 fast branch of the cell and list kernels is Lennard-Jones arithmetic: with another potential
+        // the window must stay empty (md_set_potential), or in-range pairs would silently get LJ forces
+        if (s->pot_kind != MD_POT_LJ) return MD_EINVAL;
         s->pp.precise_r2 = value;
         s->precise_r2_user = true;
     } else if (!strcmp(key, "ap_general")) {
@@ -796,14 +812,35 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
     } else if (!strcmp(key, "cell_order")) {
         // 1 = cells numbered along a Morton curve (measurement; dense kernel only: it selects "cell_kernel" = 3)
         if (value != 0 && value != 1) return MD_EINVAL;
-        s->grid.morton = (int)value;
-        s->grid.nid = s->grid.ncells;
-        if (s->grid.morton) {
-            int P = 1;
-            while (P < s->grid.n) P <<= 1;
-            s->grid.nid = P * P * P;
-            s->cell_kernel = 3;
+        if (value == 1 && !s->grid.n) return MD_EDOMAIN;
+        if (value == 1 && morton_ids(s->grid.n) > s->cell_cap) {
+            // the cell arrays were sized for n^3 ids at md_create: make room for the padded cube
+            const int nid = morton_ids(s->grid.n);
+            const int nscan = nid > s->ap_sort_bins ? nid : s->ap_sort_bins;
+            const int scan_cap = nscan / 2048 + 2;
+            CK(cudaStreamSynchronize(s->stream));
+            int *cc = (int *)ljmd_dev_alloc((size_t)nid * sizeof(int), s->stream);
+            int *cs = (int *)ljmd_dev_alloc(((size_t)nid + 1) * sizeof(int), s->stream);
+            unsigned long long *ss = (unsigned long long *)ljmd_dev_alloc((size_t)scan_cap * sizeof(unsigned long long), s->stream);
+            if (!cc || !cs || !ss) {
+                ljmd_dev_free(cc, s->stream); ljmd_dev_free(cs, s->stream); ljmd_dev_free(ss, s->stream);
+                return MD_ENOMEM;
+            }
+            ljmd_dev_free(s->cell_count, s->stream);
+            ljmd_dev_free(s->cell_start, s->stream);
+            ljmd_dev_free(s->scan_state, s->stream);
+            s->cell_count = cc;
+            s->cell_start = cs;
+            s->scan_state = ss;
+            s->cell_cap = nid;
+            s->scan_cap = scan_cap;
+            CK(cudaMemsetAsync(s->scan_state, 0, (size_t)scan_cap * sizeof(unsigned long long), s->stream));   // 0 = never written
+            ljmd_drop_graphs(s);
         }
+        s->cell_order = (int)value;
+        s->grid.morton = (int)value;
+        s->grid.nid = s->grid.morton ? morton_ids(s->grid.n) : s->grid.ncells;
+        if (s->grid.morton) s->cell_kernel = 3;
         s->layout = LAYOUT_NONE;
         s->forces_valid = false;
         CK(cudaMemsetAsync(s->cell_count, 0, (size_t)s->grid.nid * sizeof(int), s->stream));
@@ -817,7 +854,7 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
         if (value < 1) return MD_EINVAL;
         s->sort_every = (int)value;
     } else return MD_EINVAL;
-    drop_graphs(s);
+    ljmd_drop_graphs(s);
     return MD_OK;
 }
 
@@ -848,6 +885,9 @@ extern "C" int md_get_stat(md_sim *s, const char *key, double *value)
     else if (!strcmp(key, "t_other_ms")) *value = s->t_phase[TAG_OTHER];
     else if (!strcmp(key, "t_force2_ms")) *value = s->t_phase[TAG_FORCE2];
     else if (!strcmp(key, "nbr_cap")) *value = s->nbr_cap;
+    else if (!strcmp(key, "cell_order")) *value = s->grid.morton;
+    else if (!strcmp(key, "cell_ids")) *value = s->grid.nid;
+    else if (!strcmp(key, "precise_r2")) *value = s->pp.precise_r2;
     else if (!strcmp(key, "n_force")) *value = (double)s->n_phase[TAG_FORCE];
     else if (!strcmp(key, "max_occupancy")) {
         unsigned long long h = 0;

@@ -63,13 +63,17 @@ __device__ __forceinline__ float vl_local(float &x, int c, const Grid &g)
 __global__ void __launch_bounds__(1) k_vl_decide(VlCtl *ctl, unsigned thr_bits)
 {
     const unsigned m = ctl->maxd2;
-    const int rb = (m > thr_bits || ctl->force) ? 1 : 0;
+    const int asked = ctl->force;                        // set by the host only (vl_force_build)
+    const int rb = (m > thr_bits || asked) ? 1 : 0;
     ctl->rebuild = rb;
     ctl->force = 0;
     ctl->maxd2 = 0u;
     if (rb) {
         ctl->nbuilds++;
-        ctl->overflow = 0;                               // every list is rewritten: the build reports afresh
+        // `overflow` is sticky across the builds the device decides on its own: md_step reads it once, after all
+        // steps, and a list truncated in the middle of the run must still be reported even if a later build
+        // fitted.  Only a build the host asked for (after md_set_state, a grow, another path) starts afresh.
+        if (asked) ctl->overflow = 0;
     }
     ctl->nsteps++;
 }
@@ -460,6 +464,7 @@ int ljmd_vl_grow(md_sim *s, int need)
     ljmd_dev_free(s->vl_list, s->stream);
     s->vl_list = nl;
     s->vl_cap = cap;
+    ljmd_drop_graphs(s);                                 // captured build and force kernels hold the old pointer and capacity
     s->layout = LAYOUT_NONE;                             // forces a build at the next evaluation
     return MD_OK;
 }

@@ -6,6 +6,7 @@ import pytest
 
 import oracle
 from helpers import force_check
+from paper_0709_3225_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
@@ -82,3 +83,47 @@ def test_atoms_on_cell_faces_and_box_boundary(b):
 def test_rand48_zero_sized_requests(b):
     out, seeds = b.rand48([0x1234ABCD330E], 0, b.R48_U32_HI32)
     assert out.shape == (1, 0) and int(seeds[0]) == 0x1234ABCD330E
+
+
+def test_morton_numbering_survives_a_later_grid_option(b):
+    """"skin" / "cell_skin" rebuild the cell grids; the numbering chosen with "cell_order" must stay in force
+    (a bench line labelled Morton would otherwise measure the linear numbering), with the oracle's forces."""
+    pos, L = wl.perturbed_fcc(8, 0.8, 0.1, seed=31)
+    Fo, _, _ = oracle.forces(pos.astype(np.float64), L, algo=0)
+    with b.Sim(pos.shape[0], L) as s:
+        n = int(s.stat("ncell"))
+        s.option("cell_order", 1)
+        assert s.stat("cell_order") == 1 and s.stat("cell_ids") == 8 ** 3 and n ** 3 < 8 ** 3
+        s.option("skin", 0.4)
+        assert s.stat("cell_order") == 1 and s.stat("cell_ids") == 8 ** 3
+        s.set_state(pos, np.zeros_like(pos))
+        s.compute_forces(b.MD_CELL)
+        assert force_check(s.forces(), Fo)[0] == 0
+        s.step(4, b.MD_CELL)
+        s.option("cell_order", 0)
+        assert s.stat("cell_order") == 0 and s.stat("cell_ids") == n ** 3
+        s.compute_forces(b.MD_CELL)
+        p, _ = s.get_state()
+        Fo2, _, _ = oracle.forces(p.astype(np.float64), L, algo=0)
+        assert force_check(s.forces(), Fo2)[0] == 0
+
+
+def test_md_create_sizes_the_cell_arrays_for_the_linear_numbering(b):
+    """A sparse box of 260 cells per side: 2 x 70 MB of cell arrays (plus 430 MB of per-row energy partials), not
+    the 2 x 537 MB of the padded Morton cube (512^3 ids), which is allocated only when "cell_order" = 1 asks for it."""
+    import torch
+    L = 2.5 * 260 + 1.0
+    pos = (np.random.default_rng(5).random((1000, 3)) * L).astype(np.float32)
+    torch.cuda.synchronize()
+    before = torch.cuda.memory_allocated()
+    with b.Sim(pos.shape[0], L) as s:
+        assert s.stat("ncell") == 260
+        used = torch.cuda.memory_allocated() - before
+        assert used < 700e6, used
+        s.option("cell_order", 1)
+        assert torch.cuda.memory_allocated() - before > 1400e6
+        s.set_state(pos, np.zeros_like(pos))
+        s.compute_forces(b.MD_CELL)
+        F3 = s.forces()
+    Fo, _, _ = oracle.forces(pos.astype(np.float64), L, algo=0)
+    assert force_check(F3, Fo)[0] == 0

@@ -80,3 +80,24 @@ def test_md_set_potential_arguments(b):
                 s.potential(*bad)
             assert e.value.code == b.MD_EINVAL
     assert b._lib.md_set_potential(None, 0, 0.0, 0.0) == b.MD_EINVAL
+
+
+def test_fp32_window_cannot_be_reopened_under_another_potential(b):
+    """"precise_r2" opens the FP32 branch of the cell and list kernels, which is Lennard-Jones arithmetic: with the
+    Yukawa pair set it is refused, so in-range pairs can never silently get LJ forces; back on LJ it is accepted."""
+    pos, L = wl.perturbed_fcc(6, 0.8, 0.10, seed=706)
+    with oracle.potential(1, A, KAPPA):
+        Fo, _, _ = oracle.forces(pos.astype(np.float64), L, mode=1, algo=0)
+    with b.Sim(pos.shape[0], L) as s:
+        s.potential(b.MD_POT_YUKAWA, A, KAPPA)
+        with pytest.raises(b.MDError) as e:
+            s.option("precise_r2", 1.3)
+        assert e.value.code == b.MD_EINVAL
+        assert s.stat("precise_r2") > 1e100
+        s.set_state(pos, np.zeros_like(pos))
+        for algo in (b.MD_CELL, b.MD_VERLET):
+            s.compute_forces(algo)
+            assert force_check(s.forces(), Fo)[0] == 0
+        s.potential(b.MD_POT_LJ)
+        s.option("precise_r2", 1.3)
+        assert s.stat("precise_r2") == 1.3

@@ -257,3 +257,54 @@ def test_fused_integrator_of_the_list_path(b, c1, fuse, graph, chunks):
         assert force_check(s.forces(), Fo)[0] == 0
         assert s.stat("vl_steps") == 101 and 3 <= s.stat("vl_builds") <= 40
         assert ke == pytest.approx(oracle.kinetic_energy(v.astype(np.float64)), rel=1e-9)
+
+
+def test_lists_grown_after_graphs_were_captured(b):
+    """A handle that has already replayed CUDA graphs of the list path, then receives a denser state whose lists
+    outgrow the capacity: the reallocation must also forget those graphs (their nodes hold the old list pointer
+    and capacity).  Uniform state, 10 steps; clustered state (600 atoms in one cell), 10 steps; oracle forces."""
+    g = np.stack(np.meshgrid(np.arange(10), np.arange(10), np.arange(6), indexing="ij"), -1).reshape(-1, 3)
+    L = 45.5
+    uniform = (2.0 + 4.3 * g).astype(np.float32)                  # every pair beyond rc: nothing moves
+    clustered = (15.2 + 0.95 * g).astype(np.float32)
+    with b.Sim(g.shape[0], L) as s:
+        s.set_state(uniform, np.zeros_like(uniform))
+        s.step(10, b.MD_VERLET)
+        assert s.stat("graph_replays") > 0
+        cap0 = s.stat("vl_cap")
+        s.set_state(clustered, np.zeros_like(clustered))
+        s.step(10, b.MD_VERLET)
+        assert s.stat("vl_cap") > cap0 and s.stat("vl_overflow") == 0
+        p, _ = s.get_state()
+        F = s.forces()
+        _, pe, w = s.energies()
+    Fo, peo, wo = oracle.forces(p.astype(np.float64), L, algo=0)
+    assert force_check(F, Fo)[0] == 0
+    assert pe == pytest.approx(peo, rel=1e-6) and w == pytest.approx(wo, rel=1e-6)
+
+
+def test_overflow_in_the_middle_of_a_run_is_reported(b):
+    """A block of 1000 atoms contracting onto its centre and bouncing back: the builds around step 100 need lists
+    of ~100 entries (capacity 40), the builds at the end of the 400 steps fit again.  md_step reads the flag once,
+    at its end: it must still answer MD_ENOMEM (lists "are never truncated silently"), and the run repeated on the
+    enlarged lists must succeed and give the oracle's forces."""
+    n, a, alpha, L = 10, 1.3, 0.5, 45.5
+    g = np.stack(np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij"), -1).reshape(-1, 3)
+    pos = (L / 2 + a * (g - (n - 1) / 2)).astype(np.float32)
+    vel = (-alpha * (pos - np.float32(L / 2))).astype(np.float32)
+    with b.Sim(pos.shape[0], L) as s:
+        s.set_state(pos, vel)
+        s.compute_forces(b.MD_VERLET)
+        cap0 = s.stat("vl_cap")
+        assert s.stat("vl_overflow") == 0 and cap0 < 60            # the start fits
+        with pytest.raises(b.MDError) as e:
+            s.step(400, b.MD_VERLET)
+        assert e.value.code == b.MD_ENOMEM
+        assert s.stat("vl_cap") > 80                                 # enlarged for the longest list any build asked for
+        s.set_state(pos, vel)
+        s.step(400, b.MD_VERLET)
+        assert s.stat("vl_overflow") == 0
+        p, _ = s.get_state()
+        F = s.forces()
+    Fo, _, _ = oracle.forces(p.astype(np.float64), L, algo=0)
+    assert force_check(F, Fo)[0] == 0
