@@ -19,10 +19,13 @@ def melt(pos, vel, L, steps, oracle, **kw):
     return p, v.astype(np.float32)
 
 
-def check_forces(F, Fo, pos, L, oracle, rc=2.5, max_atoms=200):
-    """R15 on every component of a whole system.  A component may miss it only on an atom that has a partner
-    inside the cutoff window of R16 (|r^2/rc^2 - 1| < 4e-7, listed by the oracle through its linked cells:
-    either classification is correct there), and then by at most the force jump at the cutoff, 0.039.
+def check_forces(F, Fo, pos, L, oracle, rc=2.5, max_atoms=200, eps=1.0, sigma=1.0):
+    """R15 on every component of a whole system, with the excuse of R16 read per component:
+    a pair with |r^2/rc^2 - 1| < 4e-7 (listed by the oracle through its linked cells) may be classified either
+    way, so on an atom of such a pair the GPU force may differ from the oracle's by exactly that pair's own term
+    at the cutoff, -(f_LJ(rc)/r) d: removed if the oracle counted the pair, added if it did not.  A component that
+    misses R15 is accepted only if, for some choice of which flagged pairs of that atom were classified the other
+    way, the residual is back inside R15 on all three components.  Modes 0 and 1 (mode 2 has no jump at rc).
     Returns the number of atoms excused that way."""
     F = np.asarray(F, dtype=np.float64)
     tol = np.maximum(1e-4 * np.abs(Fo), 1e-5)
@@ -31,12 +34,28 @@ def check_forces(F, Fo, pos, L, oracle, rc=2.5, max_atoms=200):
     assert len(atoms) <= max_atoms, "too many violations: %d components" % len(bad)
     if not atoms:
         return 0
-    pairs, n = oracle.near_cutoff_pairs_cell(np.asarray(pos, dtype=np.float64), L, rc=rc, tol=4e-7, cap=1 << 20)
+    x = np.asarray(pos, dtype=np.float64)
+    pairs, n = oracle.near_cutoff_pairs_cell(x, L, rc=rc, tol=4e-7, cap=1 << 20)
     assert n <= (1 << 20)
-    flagged = set(int(i) for i in pairs[:, 0])
     for a in atoms:
-        assert a in flagged, ("R15 violated on atom %d without a near-cutoff partner" % a, F[a], Fo[a])
-        assert np.max(np.abs(F[a] - Fo[a])) < 0.04 + 1e-4, (a, F[a], Fo[a])
+        partners = [int(j) for j in pairs[pairs[:, 0] == a, 1]]
+        assert partners, ("R15 violated on atom %d without a near-cutoff partner" % a, F[a], Fo[a])
+        assert len(partners) <= 8
+        terms = []
+        for j in partners:
+            d = x[j] - x[a]
+            d -= L * np.rint(d / L)
+            r2 = float(d @ d)
+            _, _, fr = oracle.lj_pair(0, r2, eps, sigma, 1.01 * rc)      # the untruncated f/r at this distance
+            sign = -1.0 if r2 < rc * rc else 1.0                         # oracle counted it: the GPU may have dropped it
+            terms.append(sign * (-fr) * d)                               # Eq. 1: F_a -= (f/r) d
+        ok = False
+        for mask in range(1, 1 << len(terms)):
+            resid = F[a] - Fo[a] - sum(t for k, t in enumerate(terms) if mask >> k & 1)
+            if np.all(np.abs(resid) <= tol[a]):
+                ok = True
+                break
+        assert ok, ("atom %d: deviation is not the cutoff term of its near-cutoff pairs" % a, F[a], Fo[a], terms)
     return len(atoms)
 
 
