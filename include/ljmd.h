@@ -241,6 +241,12 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
 int md_set_option(md_sim *s, const char *key, double value);
 int md_get_stat(md_sim *s, const char *key, double *value);
 
+/* Calibration helper for the benchmark, not part of the MD path: the FP32 FMA rate of the current device in
+ * TFLOP/s (2 flop per FFMA), measured with a register-only kernel of independent FFMA chains at full occupancy,
+ * best of three launches timed with CUDA events on cuda_stream; *ms (may be NULL) receives that launch's time.
+ * bench.py reports it beside the derived "alu" peak (SMs x 128 lanes x 2 x max SM clock).  Allocates nothing. */
+int md_probe_fp32_peak(double *tflops, double *ms, void *cuda_stream);
+
 /* Text of the last CUDA error seen by this thread's library calls ("" if none). */
 const char *md_last_cuda_error(void);
 

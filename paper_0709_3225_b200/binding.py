@@ -53,6 +53,7 @@ _SIGS = {
     "md_get_stat": ([_vp, ctypes.c_char_p, _pd], _i32),
     "md_last_cuda_error": ([], ctypes.c_char_p),
     "rand48_kernel_launches": ([], _i64),
+    "md_probe_fp32_peak": ([_pd, _pd, _vp], _i32),
     "md_forces_allpairs_static": ([_vp, _i64, _d, _d, _d, _d, _i32, _vp, _vp, _vp], _i32),
 }
 for _name, (_args, _res) in _SIGS.items():
@@ -209,6 +210,14 @@ def md_forces_allpairs_static(pos, N, L, rc, eps, sigma, shifted, forces, pe_vir
     st = current_stream() if stream is None else int(stream)
     _check(_lib.md_forces_allpairs_static(_addr(pos), N, L, rc, eps, sigma, shifted, _addr(forces), _addr(pe_virial),
                                           st), "md_forces_allpairs_static")
+
+
+def md_probe_fp32_peak(stream=None):
+    """(TFLOP/s, ms) of the library's FFMA-chain calibration kernel on the current device."""
+    tf, ms = _d(), _d()
+    st = current_stream() if stream is None else int(stream)
+    _check(_lib.md_probe_fp32_peak(ctypes.byref(tf), ctypes.byref(ms), st), "md_probe_fp32_peak")
+    return tf.value, ms.value
 
 
 def use_torch_allocator():

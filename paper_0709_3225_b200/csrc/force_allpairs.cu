@@ -628,7 +628,7 @@ int ljmd_forces_allpairs(md_sim *s)
         int niblk = (N + AP_T - 1) / AP_T;
         int nsplit = s->ap_nsplit;
         int jchunk = (N + nsplit - 1) / nsplit;
-        jchunk = ((jchunk + AP_T - 1) / AP_T) * AP_T;
+        jchunk = (jchunk + 31) / 32 * 32;
         dim3 grid(niblk, nsplit);
         k_force_allpairs_general<<<grid, AP_T, 0, s->stream>>>(s->pos, N, s->pp, s->Lf, 1.0f / s->Lf, s->L, 1.0 / s->L,
                                                               jchunk, s->fpart, ppe, pw);

@@ -274,7 +274,9 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     const int AP_T = 128;
     int niblk = (int)((N + AP_T - 1) / AP_T);
     int nsplit = (592 + niblk - 1) / niblk;
-    if (nsplit > niblk) nsplit = niblk;
+    // j chunks are multiples of 32 atoms, whatever the number of i blocks: a small system (below
+    // N ~ 4000 the launch overhead rivals the computation) still spreads over many SMs, N = 500 over 64 blocks
+    if (nsplit > (int)((N + 31) / 32)) nsplit = (int)((N + 31) / 32);
     if (nsplit > 64) nsplit = 64;
     if (nsplit < 1) nsplit = 1;
     s->ap_nsplit = nsplit;
