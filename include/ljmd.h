@@ -111,7 +111,10 @@ int md_get_energies(md_sim *s, double *KE, double *PE, double *virial);
  * stream s.  kind: 0 uint32 x>>16; 1 uint32 x>>17 (lrand48); 2 double x*2^-48; 3 uint64 x.
  * Streams are split across warps by O(log k) skip-ahead (Eq. 6-7 with
  * R5), so nstreams = 1 with a large ndraws runs on the whole GPU.  seeds and out may each be
- * host or device memory.  ndraws = 0 or nstreams = 0 is MD_OK and writes nothing. */
+ * host or device memory.  ndraws = 0 or nstreams = 0 is MD_OK and writes nothing.
+ * MD_EINVAL for a seed with bits above 47 (host seeds are checked before anything runs; device seeds by the
+ * generating kernel itself, so the answer comes at the end of the call): no seed is changed, the contents of
+ * `out` are then unspecified. */
 int rand48_fill(uint64_t *seeds, int64_t nstreams, int64_t ndraws, int kind, void *out);
 
 /* Human-readable name of a status code; never NULL. */

@@ -11,21 +11,12 @@
 #define R48_C 0xBULL
 #define R48_MASK 0xFFFFFFFFFFFFULL
 #define R48_T 256
+#define R48_TARGET_WARPS (148 * 64 * 4)
 
-__device__ uint64_t g_r48_A[48];   // A_{2^b}
-__device__ uint64_t g_r48_C[48];   // C_{2^b}
-
-// (A, C)_{2^(b+1)} = (A, C)_{2^b} composed with itself: (A^2, A C + C).
-__global__ void k_r48_init_table()
-{
-    uint64_t a = R48_A, c = R48_C;
-    for (int b = 0; b < 48; b++) {
-        g_r48_A[b] = a;
-        g_r48_C[b] = c;
-        c = (a * c + c) & R48_MASK;
-        a = (a * a) & R48_MASK;
-    }
-}
+// The maps (A, C)_{2^b}, b < 48, in constant memory: every lane of a warp walks the bits of its skip distance in
+// the same order, so each table read is one broadcast from the constant cache (they were global loads before).
+__constant__ uint64_t g_r48_A[48];   // A_{2^b}
+__constant__ uint64_t g_r48_C[48];   // C_{2^b}
 
 // State after n further draws, by applying the power-of-two maps for the set bits of n.
 __device__ __forceinline__ uint64_t r48_skip(uint64_t x, uint64_t n)
@@ -46,6 +37,8 @@ template <> struct R48Out<2> {
 };
 template <> struct R48Out<3> { typedef uint64_t T; static __device__ __forceinline__ T cv(uint64_t x) { return x; } };
 
+__device__ int g_r48_flag;           // set by a kernel that met a seed with bits above 47; read and cleared by the host
+
 // One warp per (stream, segment).  Lane l keeps 4 states whose positions inside the current
 // 128-draw window are pos[k]; every iteration applies (A_128, C_128) to all four.
 template <int KIND>
@@ -59,6 +52,11 @@ k_rand48_fill(const uint64_t *__restrict__ seeds, int64_t nstreams, int64_t ndra
     const int64_t gw = ((int64_t)blockIdx.x * R48_T + threadIdx.x) >> 5;
     if (gw >= nstreams * nseg) return;
     const int64_t s = gw / nseg, g = gw - s * nseg;
+    const uint64_t seed = seeds[s];
+    if (seed >> 48) {                                  // not a 48-bit state: the call fails (argument check, folded in)
+        if (lane == 0) g_r48_flag = 1;
+        return;
+    }
     const int64_t start = g * seg;
     const int64_t len = min(seg, ndraws - start);
     T *out = (T *)out_ + (s * ndraws + start);
@@ -66,7 +64,7 @@ k_rand48_fill(const uint64_t *__restrict__ seeds, int64_t nstreams, int64_t ndra
     const uint64_t A128 = g_r48_A[7], C128 = g_r48_C[7];
     uint64_t st[4];
     int pos[4];
-    st[0] = r48_skip(seeds[s], (uint64_t)(start + lane * V + 1));
+    st[0] = r48_skip(seed, (uint64_t)(start + lane * V + 1));
     pos[0] = lane * V;
 #pragma unroll
     for (int k = 1; k < V; k++) {
@@ -114,11 +112,10 @@ k_rand48_fill(const uint64_t *__restrict__ seeds, int64_t nstreams, int64_t ndra
 __global__ void __launch_bounds__(R48_T)
 k_rand48_advance(uint64_t *__restrict__ seeds, int64_t nstreams, uint64_t ndraws)
 {
+    if (g_r48_flag) return;                            // the fill kernel refused a seed: no state moves
     int64_t s = (int64_t)blockIdx.x * R48_T + threadIdx.x;
     if (s < nstreams) seeds[s] = r48_skip(seeds[s], ndraws);
 }
-
-__device__ int g_r48_flag;
 
 __global__ void __launch_bounds__(R48_T)
 k_rand48_validate(const uint64_t *__restrict__ seeds, int64_t nstreams)
@@ -139,10 +136,18 @@ static int r48_ensure_table(cudaStream_t st)
     CK(cudaGetDevice(&dev));
     if (dev < 0 || dev >= 64) return MD_EUNSUPPORTED;
     if (ready[dev]) return MD_OK;
-    k_r48_init_table<<<1, 1, 0, st>>>();
-    CK(cudaGetLastError());
-    CK(cudaStreamSynchronize(st));
-    g_r48_launches++;
+    // (A, C)_{2^(b+1)} = (A, C)_{2^b} composed with itself: (A^2, A C + C)
+    uint64_t hA[48], hC[48];
+    uint64_t a = R48_A, c = R48_C;
+    for (int b = 0; b < 48; b++) {
+        hA[b] = a;
+        hC[b] = c;
+        c = (a * c + c) & R48_MASK;
+        a = (a * a) & R48_MASK;
+    }
+    CK(cudaMemcpyToSymbolAsync(g_r48_A, hA, sizeof(hA), 0, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyToSymbolAsync(g_r48_C, hC, sizeof(hC), 0, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));                     // hA, hC are on the stack; later calls may use other streams
     ready[dev] = true;
     return MD_OK;
 }
@@ -185,18 +190,24 @@ extern "C" int rand48_fill_on(uint64_t *seeds, int64_t nstreams, int64_t ndraws,
     void *dout = out;
     int rc = MD_OK;
 
-    // seeds must be 48-bit states (argument check): on the host for host arrays, by a
-    // one-pass kernel and a 4-byte flag for device arrays
-    if (seeds_dev) {
+    // seeds must be 48-bit states (argument check): on the host for host arrays.  For device arrays the fill kernel
+    // itself checks the seed it reads (a warp that meets a bad one stores nothing and raises g_r48_flag, the advance
+    // kernel then leaves every state alone) and the flag comes back with the synchronisation that ends the call:
+    // no separate validation pass, copy and synchronisation in front of the fill.  On MD_EINVAL the seeds are
+    // unchanged and the contents of `out` are unspecified.  Only a call with nothing to draw validates by itself.
+    if (seeds_dev && ndraws == 0) {
         int flag = 0;
-        CK(cudaMemcpyToSymbolAsync(g_r48_flag, &flag, sizeof(int), 0, cudaMemcpyHostToDevice, st));
         k_rand48_validate<<<(unsigned)((nstreams + R48_T - 1) / R48_T), R48_T, 0, st>>>(seeds, nstreams);
         CK(cudaGetLastError());
         g_r48_launches++;
         CK(cudaMemcpyFromSymbolAsync(&flag, g_r48_flag, sizeof(int), 0, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
-        if (flag) return MD_EINVAL;
-    } else {
+        if (flag) {
+            const int zero = 0;
+            CK(cudaMemcpyToSymbol(g_r48_flag, &zero, sizeof(int)));
+            return MD_EINVAL;
+        }
+    } else if (!seeds_dev) {
         for (int64_t i = 0; i < nstreams; i++)
             if (seeds[i] >> 48) return MD_EINVAL;
     }
@@ -217,9 +228,11 @@ extern "C" int rand48_fill_on(uint64_t *seeds, int64_t nstreams, int64_t ndraws,
         if (!dout) { rc = MD_ENOMEM; goto done; }
     }
     {
-        // segment length: a multiple of 128 draws, at least 1024, sized for ~128K warps
+        // segment length: a multiple of 128 draws, at least 1024, sized for about four waves of resident warps
+        // (148 SMs x 64): a warp pays its skip-ahead (one table step per set bit of its start, up to 28 for the
+        // 2^28-draw stream) once per segment, so few long segments beat many short ones
         int64_t total = nstreams * ndraws;
-        int64_t seg = (total / 131072 + 127) / 128 * 128;
+        int64_t seg = (total / R48_TARGET_WARPS + 127) / 128 * 128;
         if (seg < 1024) seg = 1024;
         int64_t nd128 = (ndraws + 127) / 128 * 128;
         if (seg > nd128) seg = nd128;
@@ -249,8 +262,18 @@ extern "C" int rand48_fill_on(uint64_t *seeds, int64_t nstreams, int64_t ndraws,
             e = cudaMemcpyAsync(seeds, dseeds, (size_t)nstreams * 8, cudaMemcpyDeviceToHost, st);
             if (e != cudaSuccess) { ljmd_note_cuda_error(e, "seed download", __FILE__, __LINE__); rc = MD_ECUDA; goto done; }
         }
+        int flag = 0;
+        if (seeds_dev) {
+            e = cudaMemcpyFromSymbolAsync(&flag, g_r48_flag, sizeof(int), 0, cudaMemcpyDeviceToHost, st);
+            if (e != cudaSuccess) { ljmd_note_cuda_error(e, "seed flag", __FILE__, __LINE__); rc = MD_ECUDA; goto done; }
+        }
         e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) { ljmd_note_cuda_error(e, "rand48_fill sync", __FILE__, __LINE__); rc = MD_ECUDA; }
+        else if (flag) {
+            const int zero = 0;
+            cudaMemcpyToSymbol(g_r48_flag, &zero, sizeof(int));
+            rc = MD_EINVAL;
+        }
     }
 done:
     if (!seeds_dev && dseeds) { cudaStreamSynchronize(st); ljmd_dev_free(dseeds, st); }

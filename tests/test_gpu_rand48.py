@@ -61,6 +61,17 @@ def test_device_buffers_and_unaligned_output(b):
     assert np.array_equal(dseeds.cpu().numpy().view(np.uint64), rs)
     bad = torch.tensor([1 << 50], dtype=torch.int64, device="cuda")
     assert b._lib.rand48_fill(bad.data_ptr(), 1, 4, 0, out.data_ptr()) == b.MD_EINVAL
+    assert b._lib.rand48_fill(bad.data_ptr(), 1, 0, 0, out.data_ptr()) == b.MD_EINVAL         # nothing to draw: still checked
+    # device seeds are checked by the fill kernel itself: one bad seed among good ones fails the call, no state moves,
+    # and the next call is clean
+    mixed = np.array([5, 1 << 48, 7, 9], dtype=np.uint64)
+    dm = torch.from_numpy(mixed.astype(np.int64)).cuda()
+    assert b._lib.rand48_fill(dm.data_ptr(), 4, 3000, 0, out.data_ptr()) == b.MD_EINVAL
+    assert np.array_equal(dm.cpu().numpy().view(np.uint64), mixed)
+    b.rand48_fill(dseeds.data_ptr(), 6, nd, 0, out.data_ptr())
+    ref2, rs2 = oracle.rand48_fill(rs, nd, 0)
+    assert np.array_equal(out.cpu().numpy().view(np.uint32).reshape(6, nd), ref2)
+    assert np.array_equal(dseeds.cpu().numpy().view(np.uint64), rs2)
 
 
 def test_single_stream_skip_ahead_2p24(b):
