@@ -220,6 +220,11 @@ int md_set_allocator(md_alloc_fn alloc, md_free_fn free_);
  *                    "skin" / "cell_skin" options.  The cell arrays are sized for n^3 ids at md_create and
  *                    enlarged to the padded cube (up to 8 n^3) only here: MD_ENOMEM if that fails,
  *                    MD_EDOMAIN without a cell grid
+ *   "deterministic"  1 = MD_CELL (rebuilt every step, kernels 2 and 3): after every build each cell is re-ordered by
+ *                    atom id, so forces are summed in the same order in every run and reruns are bit-identical
+ *                    (the ranks inside a cell otherwise come from an atomicAdd and the last bits of a force vary
+ *                    from run to run).  A debugging aid for parity failures: one more pass over the state per
+ *                    step; default 0.  The all-pairs and neighbour-list paths have no such option
  *   "fuse_integrator" 1 = interior steps of md_step(MD_CELL) integrate in the force kernel's epilogue
  *                    (kernels 2 and 3; default 0: measured slower)
  *   "sort_every"     all-pairs path: re-sort atoms along the Hilbert curve every k steps (default 10)

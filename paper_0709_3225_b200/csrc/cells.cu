@@ -304,6 +304,29 @@ k_scatter3(const float4 *__restrict__ pos, const float4 *__restrict__ vel, int N
     }
 }
 
+// Option "deterministic": the rank of an atom inside its cell comes from an atomicAdd, so the slot order inside a
+// cell -- and with it the order in which a force is summed, i.e. its last bits -- differs from run to run.  This
+// pass re-orders every cell by the caller's atom id (carried in pos.w): rank = number of atoms of the same cell with
+// a smaller id, O(occupancy^2) reads per cell out of L1/L2.  A debugging aid (bit-identical reruns), off by default.
+__global__ void __launch_bounds__(CB_T)
+k_order_cells(const float4 *__restrict__ pos, const float4 *__restrict__ vel, const float4 *__restrict__ lpos, int N, Grid g,
+              const int *__restrict__ cell_start, float4 *__restrict__ pos2, float4 *__restrict__ vel2,
+              float4 *__restrict__ lpos2)
+{
+    int i = blockIdx.x * CB_T + threadIdx.x;
+    if (i >= N) return;
+    const float4 p = pos[i];
+    const int c = cell_id(cell_coord(p.x, g), cell_coord(p.y, g), cell_coord(p.z, g), g);
+    const int beg = cell_start[c], end = cell_start[c + 1];
+    const int id = __float_as_int(p.w);
+    int rank = 0;
+    for (int j = beg; j < end; j++) rank += (__float_as_int(pos[j].w) < id) ? 1 : 0;
+    const int dst = beg + rank;
+    pos2[dst] = p;
+    vel2[dst] = vel[i];
+    if (lpos) lpos2[dst] = lpos[i];
+}
+
 int ljmd_kick_drift_bin3(md_sim *s, int kicks)
 {
     int N = (int)s->N;
@@ -342,6 +365,15 @@ int ljmd_cell_build3(md_sim *s)
         float4 *t = s->pos; s->pos = s->pos2; s->pos2 = t;
     }
     float4 *t = s->vel; s->vel = s->vel2; s->vel2 = t;
+    if (s->deterministic) {
+        // pos2 and vel2 are free now (they held the pre-scatter state); the cell-local copies go to their twin
+        k_order_cells<<<nb, CB_T, 0, s->stream>>>(s->pos, s->vel, lp, N, s->grid, s->cell_start, s->pos2, s->vel2,
+                                                  lp ? s->lpos_det : nullptr);
+        CKL(s);
+        t = s->pos; s->pos = s->pos2; s->pos2 = t;
+        t = s->vel; s->vel = s->vel2; s->vel2 = t;
+        if (lp) { t = s->lpos; s->lpos = s->lpos_det; s->lpos_det = t; }
+    }
     s->layout = LAYOUT_CELL;
     return MD_OK;
 }

@@ -146,6 +146,8 @@ struct md_sim {
     bool precise_r2_user;         // "precise_r2" was set through md_set_option
     int cell_group;               // cells per row group of the cell-force kernel; 0 = automatic
     int cell_kernel;              // 2 (default): force_cell2.cu; 3: force_cell3.cu (dense); 1: force_cell.cu
+    bool deterministic;           // option "deterministic": cells re-ordered by atom id after every build (cells.cu)
+    float4 *lpos_det;             // twin of lpos for that pass (allocated when the option is switched on)
     int cell_order;               // option "cell_order" (1 = Morton numbering); re-applied to `grid` whenever it is rebuilt
     int cell_cap;                 // ints allocated for cell_count (cell_start has one more)
     bool cell_skin_on;            // option "cell_skin" > 0: MD_CELL runs on skin cells (verlet.cu)

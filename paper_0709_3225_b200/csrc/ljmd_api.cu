@@ -232,7 +232,7 @@ static void free_all(md_sim *s)
     free(s->ev_pool);
     free(s->ev_tag);
     void *ptrs[] = {s->pos, s->vel, s->frc, s->pos2, s->vel2, s->lpos, s->lpos2, s->cell_of, s->rank, s->cell_count,
-                    s->cell_start, s->max_occ, s->scan_ctl, s->scan_state, s->vl_list, s->vl_count, s->vl_lbuild, s->vl_ctl, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list, s->and_t_dev,
+                    s->cell_start, s->max_occ, s->scan_ctl, s->scan_state, s->lpos_det, s->vl_list, s->vl_count, s->vl_lbuild, s->vl_ctl, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list, s->and_t_dev,
                     s->tile_start};
     for (void *p : ptrs) ljmd_dev_free(p, st);
 }
@@ -846,6 +846,15 @@ extern "C" int md_set_option(md_sim *s, const char *key, double value)
         s->layout = LAYOUT_NONE;
         s->forces_valid = false;
         CK(cudaMemsetAsync(s->cell_count, 0, (size_t)s->grid.nid * sizeof(int), s->stream));
+    } else if (!strcmp(key, "deterministic")) {
+        if (value != 0 && value != 1) return MD_EINVAL;
+        if (value == 1 && !s->lpos_det) {
+            s->lpos_det = (float4 *)ljmd_dev_alloc((size_t)s->N * sizeof(float4), s->stream);
+            if (!s->lpos_det) return MD_ENOMEM;
+        }
+        s->deterministic = value == 1;
+        s->layout = LAYOUT_NONE;
+        s->forces_valid = false;
     } else if (!strcmp(key, "fuse_integrator")) {
         s->fuse_integrator = value != 0.0;
     } else if (!strcmp(key, "cell_kernel")) {
