@@ -81,18 +81,26 @@ k_force_allpairs_static(const float *__restrict__ pos, int N, PairParams P, floa
         }
         __syncthreads();
         if (!live) continue;
-#pragma unroll 4
-        for (int k = 0; k < cnt; k++) {
-            const float xj = tx[k], yj = ty[k], zj = tz[k];
-            float dx = xj - xi, dy = yj - yi, dz = zj - zi;
-            dx = fmaf(-L, rintf(dx * invL), dx);
-            dy = fmaf(-L, rintf(dy * invL), dy);
-            dz = fmaf(-L, rintf(dz * invL), dz);
-            const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-            if (r2 < P.rc2f_filter && (j0 + k) != i) {
+        // 32 j at a time: an FP32 pass marks the candidates in a bit mask, then every lane walks its own bits (the warp
+        // takes the long FP64 branch max-over-lanes(hits) times instead of on nearly every j)
+        for (int k0 = 0; k0 < cnt; k0 += 32) {
+            const int kn = min(32, cnt - k0);
+            unsigned hits = 0u;
+#pragma unroll 8
+            for (int k = 0; k < kn; k++) {
+                float dx = tx[k0 + k] - xi, dy = ty[k0 + k] - yi, dz = tz[k0 + k] - zi;
+                dx = fmaf(-L, rintf(dx * invL), dx);
+                dy = fmaf(-L, rintf(dy * invL), dy);
+                dz = fmaf(-L, rintf(dz * invL), dz);
+                const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                hits |= (r2 < P.rc2f_filter && (j0 + k0 + k) != i) ? (1u << k) : 0u;
+            }
+            while (hits) {
+                const int k = k0 + __ffs(hits) - 1;
+                hits &= hits - 1u;
                 // the FP32 test only has to be conservative: the pair is decided and evaluated in FP64
                 // from the coordinates as stored
-                double ex = (double)xj - (double)xi, ey = (double)yj - (double)yi, ez = (double)zj - (double)zi;
+                double ex = (double)tx[k] - (double)xi, ey = (double)ty[k] - (double)yi, ez = (double)tz[k] - (double)zi;
                 ex = fma(-Ld, rint(ex * invLd), ex);
                 ey = fma(-Ld, rint(ey * invLd), ey);
                 ez = fma(-Ld, rint(ez * invLd), ez);
