@@ -115,6 +115,7 @@ struct md_sim {
     // all-pairs partial forces: [nsplit][3][N] doubles
     double *fpart;
     int ap_nsplit;                // j splits of the general kernel
+    unsigned *ap_tile_done;       // [i blocks] arrival counters of the general kernel (zero between launches)
     // all-pairs tiled kernel: R atoms per thread, i blocks, j splits, Morton sort grid,
     // pre-shift validity bound
     bool ap_tiled, ap_force_general;

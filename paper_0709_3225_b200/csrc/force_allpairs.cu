@@ -38,10 +38,12 @@
 __global__ void __launch_bounds__(AP_T)
 k_force_allpairs_general(const float4 *__restrict__ pos, int N, PairParams P, float L, float invL,
                          double Ld, double invLd, int jchunk, double *__restrict__ fpart,
-                         double *__restrict__ part_pe, double *__restrict__ part_w)
+                         double *__restrict__ part_pe, double *__restrict__ part_w, unsigned *__restrict__ tile_done,
+                         float4 *__restrict__ frc)
 {
     __shared__ float4 tile[AP_T];
     __shared__ double red[32];
+    __shared__ int last_of_tile;
     const int tid = threadIdx.x;
     const int i = blockIdx.x * AP_T + tid;
     const int jbeg = blockIdx.y * jchunk;
@@ -101,6 +103,27 @@ k_force_allpairs_general(const float4 *__restrict__ pos, int N, PairParams P, fl
         part_pe[b] = 0.5 * pe;            // every pair is visited from both ends
         part_w[b] = 0.5 * w;
     }
+    // Combination of the j splits inside this launch (it was a kernel of its own: one launch less per step, which
+    // is what a small system's step consists of): the block that arrives last on this tile of atoms sums
+    // the tile's partial forces in split order -- the same sum whoever that is -- and puts the counter back to zero
+    // for the next launch.
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) last_of_tile = atomicAdd(&tile_done[blockIdx.x], 1u) == gridDim.y - 1;
+    __syncthreads();
+    if (!last_of_tile) return;
+    __threadfence();
+    if (live) {
+        double sx = 0.0, sy = 0.0, sz = 0.0;
+        for (int s = 0; s < (int)gridDim.y; s++) {
+            const size_t base = (size_t)s * 3 * N;
+            sx += __ldcg(&fpart[base + i]);
+            sy += __ldcg(&fpart[base + (size_t)N + i]);
+            sz += __ldcg(&fpart[base + 2 * (size_t)N + i]);
+        }
+        frc[i] = make_float4((float)sx, (float)sy, (float)sz, 0.0f);
+    }
+    if (tid == 0) tile_done[blockIdx.x] = 0u;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -478,22 +501,6 @@ k_allpairs_eval(const float4 *__restrict__ pos, int N, PairParams P, double Ld, 
     }
 }
 
-// Deterministic combine of the j-split partial forces: frc[i] = sum_s fpart[s][.][i].
-__global__ void __launch_bounds__(256)
-k_combine_forces(float4 *__restrict__ frc, const double *__restrict__ fpart, int N, int nsplit)
-{
-    int i = blockIdx.x * 256 + threadIdx.x;
-    if (i >= N) return;
-    double fx = 0.0, fy = 0.0, fz = 0.0;
-    for (int s = 0; s < nsplit; s++) {
-        size_t base = (size_t)s * 3 * N;
-        fx += fpart[base + i];
-        fy += fpart[base + (size_t)N + i];
-        fz += fpart[base + 2 * (size_t)N + i];
-    }
-    frc[i] = make_float4((float)fx, (float)fy, (float)fz, 0.0f);
-}
-
 // ---------------------------------------------------------------------------------------
 // Host side: choose R and the j split (md_create), sort, launch.
 static int ap_sm_count()
@@ -643,14 +650,11 @@ int ljmd_forces_allpairs(md_sim *s)
         jchunk = (jchunk + 31) / 32 * 32;
         dim3 grid(niblk, nsplit);
         k_force_allpairs_general<<<grid, AP_T, 0, s->stream>>>(s->pos, N, s->pp, s->Lf, 1.0f / s->Lf, s->L, 1.0 / s->L,
-                                                              jchunk, s->fpart, ppe, pw);
+                                                              jchunk, s->fpart, ppe, pw, s->ap_tile_done, s->frc);
         CKL(s);
         s->n_pe = niblk * nsplit;
         if (s->layout == LAYOUT_CELL || s->layout == LAYOUT_VERLET) s->layout = LAYOUT_NONE;   // lpos no longer tracked
         ljmd_tick(s, TAG_FORCE);
-        k_combine_forces<<<(N + 255) / 256, 256, 0, s->stream>>>(s->frc, s->fpart, N, nsplit);
-        CKL(s);
-        ljmd_tick(s, TAG_OTHER);
     }
     return MD_OK;
 }

@@ -232,7 +232,7 @@ static void free_all(md_sim *s)
     free(s->ev_pool);
     free(s->ev_tag);
     void *ptrs[] = {s->pos, s->vel, s->frc, s->pos2, s->vel2, s->lpos, s->lpos2, s->cell_of, s->rank, s->cell_count,
-                    s->cell_start, s->max_occ, s->scan_ctl, s->scan_state, s->lpos_det, s->vl_list, s->vl_count, s->vl_lbuild, s->vl_ctl, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list, s->and_t_dev,
+                    s->cell_start, s->max_occ, s->scan_ctl, s->scan_state, s->lpos_det, s->ap_tile_done, s->vl_list, s->vl_count, s->vl_lbuild, s->vl_ctl, s->fpart, s->part, s->energies, s->xfer, s->tile_count, s->nbr_count, s->nbr_list, s->and_t_dev,
                     s->tile_start};
     for (void *p : ptrs) ljmd_dev_free(p, st);
 }
@@ -313,6 +313,7 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->scan_ctl = (ScanCtl *)ljmd_dev_alloc(sizeof(ScanCtl), st);
     s->scan_state = (unsigned long long *)ljmd_dev_alloc((size_t)s->scan_cap * sizeof(unsigned long long), st);
     s->fpart = (double *)ljmd_dev_alloc((size_t)nsplit * 3 * N * sizeof(double), st);
+    s->ap_tile_done = (unsigned *)ljmd_dev_alloc((size_t)niblk * sizeof(unsigned), st);
     s->part = (double *)ljmd_dev_alloc((size_t)3 * s->part_cap * sizeof(double), st);
     s->energies = (double *)ljmd_dev_alloc(3 * sizeof(double), st);
     s->and_t_dev = (uint64_t *)ljmd_dev_alloc(sizeof(uint64_t), st);
@@ -321,12 +322,13 @@ extern "C" int md_create(md_sim **out, int64_t N, double L, double rc, double ep
     s->tile_count = (int *)ljmd_dev_alloc((size_t)ntiles * sizeof(int), st);
     s->tile_start = (int *)ljmd_dev_alloc(((size_t)ntiles + 1) * sizeof(int), st);
     if (!s->tile_count || !s->tile_start || !s->pos || !s->vel || !s->frc || !s->pos2 || !s->vel2 || !s->lpos || !s->cell_of || !s->rank ||
-        !s->cell_count || !s->cell_start || !s->max_occ || !s->scan_ctl || !s->scan_state || !s->fpart || !s->part || !s->energies || !s->xfer || !s->and_t_dev) {
+        !s->cell_count || !s->cell_start || !s->max_occ || !s->scan_ctl || !s->scan_state || !s->fpart || !s->ap_tile_done || !s->part || !s->energies || !s->xfer || !s->and_t_dev) {
         free_all(s);
         delete s;
         return MD_ENOMEM;
     }
     cudaError_t e = cudaMemsetAsync(s->cell_count, 0, (size_t)ncells * sizeof(int), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->ap_tile_done, 0, (size_t)niblk * sizeof(unsigned), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(s->max_occ, 0, sizeof(unsigned long long), st);
     if (e == cudaSuccess) {
         ScanCtl c0;
